@@ -1,0 +1,132 @@
+/* mhd.h — C ABI of the B200 (sm_100a) pseudo-spectral isothermal MHD step.
+ *
+ * What it computes (arxiv 2402.05478, PAPER.md):
+ *   eq. (1) PAPER.md:39   d rho/dt + div(rho u) = 0
+ *   eq. (2) PAPER.md:41   d(rho u)/dt + div[rho u u + (P + B^2/2) I - B B] = (1/Re) lap u   (f = 0)
+ *   eq. (3) PAPER.md:45   P = Cs^2 rho
+ *   eq. (4) PAPER.md:47   dB/dt + div(u B - B u) = (1/Rm) lap B      ( = curl(u x B) + eta lap B )
+ * discretised as PAPER.md:78 describes: Fourier pseudo-spectral on a triply periodic box [0,2pi)^3,
+ * derivatives by i*k in Fourier space, products in real space, "standard 2/3 de-aliasing rule",
+ * Adams-Bashforth time stepping (AB2 with a forward-Euler first step) or Runge-Kutta 4
+ * (Table II), double precision.  Evolved variables are rho, m = rho u
+ * and B as spectral coefficients; the caller sees rho, u, B on the grid.
+ *
+ * Everything runs on ONE GPU in hand-written CUDA kernels (own FFT; no cuFFT, no CPU fallback).
+ * The library never allocates or frees device memory: the caller passes a workspace (e.g. a torch
+ * tensor) and a CUDA stream; all work is enqueued on that stream.
+ *
+ * Layouts.  Real fields: nx*ny*nz doubles, index ((z*ny + y)*nx + x), x fastest, x_j = 2*pi*j/nx.
+ * Half-spectra (FFT entry points only): [batch][nz][ny][nx/2+1] complex, re/im interleaved,
+ * kx = 0..nx/2 fastest, ky / kz in FFT order.  Forward transform f^(k) = sum_x f(x) exp(-i k.x),
+ * unnormalised; the inverse includes 1/(nx*ny*nz).
+ *
+ * Sizes: nx, ny in {8,12,16,24,32,48,64,96,128,192,256,384,512,768,1024}; nz from the same set or
+ * nz == 1 (2-D run: the z transform is the identity and kz = 0).
+ *
+ * Pointers named *_dev are DEVICE pointers, *_host are HOST pointers (pinned memory makes the
+ * copies asynchronous, pageable memory works too).  Every call returns MHD_OK or a negative code;
+ * nothing throws, aborts or prints.  Invalid arguments are rejected before any launch.  A context
+ * is not thread-safe; distinct contexts are independent.  Results are bit-reproducible run to run
+ * (no floating-point atomics).
+ */
+#ifndef MHD_H
+#define MHD_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mhd_ctx mhd_ctx;            /* opaque; host memory owned by the library, freed by mhd_destroy */
+typedef struct mhd_fft_plan mhd_fft_plan;  /* opaque */
+
+enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ENOMEM = -2, MHD_ECUDA = -3, MHD_ESTATE = -4, MHD_ENONFINITE = -5 };
+enum { MHD_AB2 = 0, MHD_RK4 = 1 };
+enum {
+    MHD_FLAG_HYDRO = 1u,      /* B == 0 held exactly: induction and Lorentz terms skipped */
+    MHD_FLAG_NO_DEALIAS = 2u  /* keep every mode (tests only) */
+};
+
+/* mean values are volume averages <.> = (1/N) sum over the grid */
+typedef struct {
+    long long step;    /* steps taken since mhd_set_fields */
+    double time;       /* step * dt */
+    double ekin;       /* 1/2 <rho |u|^2> */
+    double emag;       /* 1/2 <|B|^2>               (eq. 2) */
+    double eiso;       /* Cs^2 <rho ln rho>: ekin+emag+eiso is the ideal invariant of the isothermal system */
+    double mass;       /* <rho> */
+    double mom[3];     /* <rho u> */
+    double bmean[3];   /* <B> */
+    double max_divb;   /* max_x |IFFT(i k . B^)| */
+} mhd_diag;
+
+/* Bytes of device workspace mhd_create needs for this configuration (0 if the size is unsupported). */
+size_t mhd_workspace_bytes(int nx, int ny, int nz, int integrator, unsigned flags);
+
+/* Create a context.  nu = 1/Re, eta = 1/Rm, cs = sound speed (all >= 0), dt > 0.
+ * workspace_dev: caller-owned device memory, 256-byte aligned, >= mhd_workspace_bytes(...), must stay
+ * alive and untouched until mhd_destroy.  cuda_stream: a cudaStream_t; NULL = the legacy default
+ * stream, on which mhd_step cannot use CUDA graphs (small grids then pay per-launch latency).
+ * Errors: MHD_EINVAL (bad size/parameter/NULL/workspace too small), MHD_ENOMEM (host), MHD_ECUDA. */
+int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, double cs, double dt,
+               int integrator, unsigned flags, void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+void mhd_destroy(mhd_ctx* ctx);
+
+/* Set the state from grid fields: m = rho*u, forward transform, 2/3 mask.
+ * Resets step count, time and integrator history.  b* may be NULL with MHD_FLAG_HYDRO.
+ * Asynchronous on the context's stream; inputs are read, never written. */
+int mhd_set_fields(mhd_ctx* ctx, const double* rho_dev, const double* ux_dev, const double* uy_dev,
+                   const double* uz_dev, const double* bx_dev, const double* by_dev, const double* bz_dev);
+/* Same from HOST arrays: copies host->device into the workspace on the stream, then as above. */
+int mhd_set_fields_host(mhd_ctx* ctx, const double* rho_host, const double* ux_host, const double* uy_host,
+                        const double* uz_host, const double* bx_host, const double* by_host, const double* bz_host);
+
+/* Advance nsteps >= 0 time steps (one RHS evaluation per AB2 step, four per RK4 step).
+ * Asynchronous: enqueues and returns.  MHD_ESTATE before the first mhd_set_fields. */
+int mhd_step(mhd_ctx* ctx, int nsteps);
+
+/* Current rho, u = m/rho, B on the grid, into caller-owned DEVICE (or HOST) arrays; b* may be NULL.
+ * The device variant is asynchronous; the host variant returns after the copies have completed. */
+int mhd_get_fields(mhd_ctx* ctx, double* rho_dev, double* ux_dev, double* uy_dev, double* uz_dev,
+                   double* bx_dev, double* by_dev, double* bz_dev);
+int mhd_get_fields_host(mhd_ctx* ctx, double* rho_host, double* ux_host, double* uy_host, double* uz_host,
+                        double* bx_host, double* by_host, double* bz_host);
+
+/* Diagnostics of the current state into HOST memory; synchronises the stream.
+ * Spectra (optional, nshell may be 0): shell s = round(|k|), s = 0..nshell-1,
+ *   ekin_spec[s] = sum_{k in s} 1/2 |u^(k)|^2 / N^2   with u = m/rho (sums to 1/2 <|u|^2>),
+ *   emag_spec[s] = sum_{k in s} 1/2 |B^(k)|^2 / N^2   (sums to emag).
+ * Returns MHD_ENONFINITE (values still filled) if a NaN/Inf or rho <= 0 was seen, MHD_ECUDA on a
+ * sticky CUDA error. */
+int mhd_diagnostics(mhd_ctx* ctx, mhd_diag* out_host, double* ekin_spec_host, double* emag_spec_host, int nshell);
+
+const char* mhd_strerror(int code);
+const char* mhd_last_error(const mhd_ctx* ctx);   /* detail of the last failure on this context ("" if none) */
+
+/* ---- FFT-only entry points (BASELINE config 5: batched 3-D R2C / C2R throughput) ---------------- */
+size_t mhd_fft_workspace_bytes(int nx, int ny, int nz, int batch);
+int  mhd_fft_plan_create(mhd_fft_plan** out, int nx, int ny, int nz, int batch,
+                         void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+/* in_real_dev: [batch][nz][ny][nx] doubles; out_complex_dev: [batch][nz][ny][nx/2+1] complex; unnormalised */
+int  mhd_fft_r2c(mhd_fft_plan* plan, const double* in_real_dev, double* out_complex_dev);
+/* inverse, includes 1/(nx*ny*nz); Im of self-conjugate x modes (kx = 0, nx/2 of a row) is ignored */
+int  mhd_fft_c2r(mhd_fft_plan* plan, const double* in_complex_dev, double* out_real_dev);
+void mhd_fft_plan_destroy(mhd_fft_plan* plan);
+
+/* number of kernel launches this library has enqueued since load (bench.py's gpu_launches) */
+long long mhd_launch_count(void);
+
+/* Per-kernel timing for the roofline report.  After mhd_profile_begin, mhd_step runs its kernels
+ * eagerly with a CUDA-event pair around every launch (on the context's stream); mhd_profile_end
+ * synchronises, fills counts[i] (launches) and ms[i] (summed device time) for the
+ * mhd_profile_kernel_count() kernel classes named by mhd_profile_kernel_name(i) -- in hot-path
+ * order: z inverse, y inverse, x C2R, products, x R2C, y forward, z forward, stage -- and switches
+ * profiling off.  Both arrays are HOST memory of that length. */
+int mhd_profile_kernel_count(void);
+const char* mhd_profile_kernel_name(int i);
+int mhd_profile_begin(mhd_ctx* ctx);
+int mhd_profile_end(mhd_ctx* ctx, int* counts_host, double* ms_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

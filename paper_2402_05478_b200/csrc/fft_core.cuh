@@ -1,0 +1,170 @@
+// fft_core.cuh — in-register / shared-memory Stockham pencil FFT for sm_100a, fp64.
+//
+// One "pencil" is a 1-D complex transform of compile-time length N (the FFT under the
+// pseudo-spectral derivative; the paper calls cuFFT/AccFFT, here it is hand-written).  Eight pencils
+// that are adjacent in memory are transformed side by side: lane = (pencil p = tid & 7,
+// slot i = tid >> 3).  A warp therefore touches 4 rows x 8 pencils x 16 B = four full 128-byte
+// lines in global memory and four conflict-free wavefronts in shared memory, for any stride.
+//
+// Each thread keeps E = N/TP elements in registers.  A pass of radix r does E/r butterflies per
+// thread; between passes the data is exchanged through one shared buffer laid out [N][8] complex.
+// Stockham auto-sort indexing (P = product of the radices already done, t = N/r):
+//     butterfly b:  k = b mod P,  inputs x[b + q*t],  twiddle w_N^(k*q*N/(P*r)),  outputs y[(b-k)*r + k + q*P]
+// so the first pass reads rows b + q*N/r0 and the last pass leaves X[b + q*N/rL] in registers,
+// which lets the callers load from and store to global memory directly, with no extra staging.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mhdfft {
+
+typedef double2 cplx;
+
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ cplx cconj(cplx a) { return make_double2(a.x, -a.y); }
+// a * (-i) for the forward transform, a * (+i) for the inverse
+template <bool INV>
+__device__ __forceinline__ cplx mul_mi(cplx a) {
+    return INV ? make_double2(-a.y, a.x) : make_double2(a.y, -a.x);
+}
+
+// ---- radix plans ---------------------------------------------------------------------------
+// radices in execution order; a factor 3, if any, goes last so that P stays a power of two.
+template <int N> struct Plan;
+#define MHD_PLAN(N_, E_, NP_, R0, R1, R2, R3)                                                    \
+    template <> struct Plan<N_> {                                                                \
+        static constexpr int E = E_;   /* elements per thread */                                 \
+        static constexpr int NP = NP_; /* passes */                                              \
+        static constexpr int TP = N_ / E_; /* threads per pencil */                              \
+        __host__ __device__ static constexpr int radix(int s) {                                  \
+            return s == 0 ? R0 : s == 1 ? R1 : s == 2 ? R2 : R3;                                 \
+        }                                                                                        \
+    };
+MHD_PLAN(8, 8, 1, 8, 1, 1, 1)
+MHD_PLAN(16, 8, 2, 8, 2, 1, 1)
+MHD_PLAN(32, 8, 2, 8, 4, 1, 1)
+MHD_PLAN(64, 8, 2, 8, 8, 1, 1)
+MHD_PLAN(128, 8, 3, 8, 4, 4, 1)
+MHD_PLAN(256, 8, 3, 8, 8, 4, 1)
+MHD_PLAN(512, 8, 3, 8, 8, 8, 1)
+MHD_PLAN(1024, 8, 4, 8, 8, 4, 4)
+MHD_PLAN(12, 12, 2, 4, 3, 1, 1)
+MHD_PLAN(24, 24, 2, 8, 3, 1, 1)
+MHD_PLAN(48, 12, 3, 4, 4, 3, 1)
+MHD_PLAN(96, 24, 3, 8, 4, 3, 1)
+MHD_PLAN(192, 24, 3, 8, 8, 3, 1)
+MHD_PLAN(384, 24, 4, 8, 4, 4, 3)
+MHD_PLAN(768, 24, 4, 8, 8, 4, 3)
+#undef MHD_PLAN
+
+// pencil groups per CTA (8 pencils each), chosen so a CTA has 128..512 threads
+template <int N> struct Tile {
+    static constexpr int TP = Plan<N>::TP;
+    static constexpr int G = (8 * TP >= 128) ? 1 : 128 / (8 * TP);
+    static constexpr int THREADS = 8 * TP * G;
+    static constexpr int COLS = 8 * G;                       // pencils per CTA
+    static constexpr size_t SMEM = (size_t)N * COLS * sizeof(cplx);
+};
+
+// ---- butterflies (natural-order outputs) ---------------------------------------------------
+template <bool INV> __device__ __forceinline__ void bfly2(cplx* v) {
+    cplx a = v[0], b = v[1];
+    v[0] = cadd(a, b); v[1] = csub(a, b);
+}
+template <bool INV> __device__ __forceinline__ void bfly4(cplx& a0, cplx& a1, cplx& a2, cplx& a3) {
+    cplx t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = mul_mi<INV>(csub(a1, a3));
+    a0 = cadd(t0, t2); a1 = cadd(t1, t3); a2 = csub(t0, t2); a3 = csub(t1, t3);
+}
+template <bool INV> __device__ __forceinline__ void bfly3(cplx* v) {
+    const double h = 0.86602540378443864676;  // sqrt(3)/2
+    cplx t = cadd(v[1], v[2]), d = csub(v[1], v[2]);
+    cplx m = make_double2(v[0].x - 0.5 * t.x, v[0].y - 0.5 * t.y);
+    cplx s = mul_mi<INV>(make_double2(h * d.x, h * d.y));   // (-/+ i) * sqrt(3)/2 * (v1 - v2)
+    v[0] = cadd(v[0], t); v[1] = cadd(m, s); v[2] = csub(m, s);
+}
+template <bool INV> __device__ __forceinline__ void bfly8(cplx* v) {
+    const double r = 0.70710678118654752440;  // 1/sqrt(2)
+    cplx e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6];
+    cplx o0 = v[1], o1 = v[3], o2 = v[5], o3 = v[7];
+    bfly4<INV>(e0, e1, e2, e3);
+    bfly4<INV>(o0, o1, o2, o3);
+    // o_k *= w8^k, w8 = exp(-/+ i pi/4)
+    cplx w1 = INV ? make_double2(r * (o1.x - o1.y), r * (o1.x + o1.y)) : make_double2(r * (o1.x + o1.y), r * (o1.y - o1.x));
+    cplx w2 = mul_mi<INV>(o2);
+    cplx w3 = INV ? make_double2(r * (-o3.x - o3.y), r * (o3.x - o3.y)) : make_double2(r * (o3.y - o3.x), r * (-o3.x - o3.y));
+    v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+    v[1] = cadd(e1, w1); v[5] = csub(e1, w1);
+    v[2] = cadd(e2, w2); v[6] = csub(e2, w2);
+    v[3] = cadd(e3, w3); v[7] = csub(e3, w3);
+}
+template <int R, bool INV> __device__ __forceinline__ void bfly(cplx* v) {
+    if constexpr (R == 8) bfly8<INV>(v);
+    else if constexpr (R == 4) bfly4<INV>(v[0], v[1], v[2], v[3]);
+    else if constexpr (R == 3) bfly3<INV>(v);
+    else if constexpr (R == 2) bfly2<INV>(v);
+}
+
+// index of the q-th input of butterfly m held by slot i in the FIRST pass, and of the q-th output in the LAST
+template <int N> __device__ __forceinline__ int first_index(int i, int m, int q) {
+    return i + Plan<N>::TP * m + q * (N / Plan<N>::radix(0));
+}
+template <int N> __device__ __forceinline__ int last_index(int i, int m, int q) {
+    return i + Plan<N>::TP * m + q * (N / Plan<N>::radix(Plan<N>::NP - 1));
+}
+// position in the register array of (butterfly m, leg q) for first / last pass
+template <int N> __device__ __forceinline__ constexpr int first_reg(int m, int q) { return m * Plan<N>::radix(0) + q; }
+template <int N> __device__ __forceinline__ constexpr int last_reg(int m, int q) { return m * Plan<N>::radix(Plan<N>::NP - 1) + q; }
+
+// ---- the passes ----------------------------------------------------------------------------
+// tw[j] = exp(-2*pi*i*j/N), j = 0..N-1 (forward); the inverse conjugates on the fly.
+// sm: this pencil group's [N][8] buffer.  i: slot in pencil (0..TP-1).  p: pencil (0..7).
+template <int N, bool INV, int S, int P>
+struct Pass {
+    static constexpr int R = Plan<N>::radix(S);
+    static constexpr int E = Plan<N>::E;
+    static constexpr int TP = Plan<N>::TP;
+    static constexpr bool LAST = (S == Plan<N>::NP - 1);
+    __device__ __forceinline__ static void run(cplx (&v)[E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
+#pragma unroll
+        for (int m = 0; m < E / R; ++m) {
+            const int b = i + TP * m;
+            const int k = b & (P - 1);
+            if constexpr (S > 0) {
+#pragma unroll
+                for (int q = 1; q < R; ++q) {
+                    cplx w = __ldg(&tw[k * q * (N / (P * R))]);
+                    if (INV) w.y = -w.y;
+                    v[m * R + q] = cmul(v[m * R + q], w);
+                }
+            }
+            bfly<R, INV>(&v[m * R]);
+            if constexpr (!LAST) {
+                const int j = (b - k) * R + k;
+#pragma unroll
+                for (int q = 0; q < R; ++q) sm[(j + q * P) * 8 + p] = v[m * R + q];
+            }
+        }
+        if constexpr (!LAST) {
+            constexpr int Rn = Plan<N>::radix(S + 1);
+            __syncthreads();
+#pragma unroll
+            for (int m = 0; m < E / Rn; ++m)
+#pragma unroll
+                for (int q = 0; q < Rn; ++q) v[m * Rn + q] = sm[(i + TP * m + q * (N / Rn)) * 8 + p];
+            __syncthreads();
+            Pass<N, INV, S + 1, P * R>::run(v, sm, i, p, tw);
+        }
+    }
+};
+
+// Transform the pencil whose first-pass inputs are in v (see first_index); on return v holds the
+// last-pass outputs (see last_index).  All threads of the CTA must call it (it synchronises).
+template <int N, bool INV>
+__device__ __forceinline__ void pencil_fft(cplx (&v)[Plan<N>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
+    Pass<N, INV, 0, 1>::run(v, sm, i, p, tw);
+}
+
+}  // namespace mhdfft

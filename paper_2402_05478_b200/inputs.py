@@ -1,6 +1,6 @@
 """Seeded synthetic inputs for the BASELINE.json configs (SURVEY.md §8(d) recipes).
 
-This module is the ONLY code shared by the CUDA path and the CPU oracle.  It holds
+This module is the ONLY code shared by the CUDA path and the CPU checker (oracle).  It holds
 none of the method's arithmetic: it only writes down initial conditions (closed
 forms from PAPER.md and seeded random-phase Fourier sums) as plain numpy arrays
 that are then handed, identically, to both sides.  numpy's FFT is used here for
