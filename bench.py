@@ -72,6 +72,7 @@ def algorithmic_bytes(g, hydro=False):
     b["fft_x_c2r"] = nin * (w2 + real)
     b["fft_x_r2c"] = nout * (real + w2)
     b["products"] = (nin + nout) * real
+    b["x_fused"] = (nin + nout) * w2                     # C2R-x + products + R2C-x in one kernel: rows in, rows out
     b["stage"] = (nout + 2 * nin + 2 * nin) * spec       # read flux + state + history, write state + history
     return b
 

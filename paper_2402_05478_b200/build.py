@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmhd_b200.so")
-SOURCES = ["fft_kernels.cu", "mhd_kernels.cu", "mhd_api.cu"]
+SOURCES = ["fft_kernels.cu", "xfused_kernel.cu", "mhd_kernels.cu", "mhd_api.cu"]
 HEADERS = ["fft_core.cuh", "mhd_internal.h"]
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -38,7 +38,8 @@ def is_stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or is_stale():
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", LIB] + \
+        extra = os.environ.get("MHD_NVCC_EXTRA", "").split()     # tuning experiments, e.g. -DMHD_XFUSED_MINBLOCKS=6
+        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", LIB] + \
               [os.path.join(CSRC, f) for f in SOURCES]
         subprocess.run(cmd, check=True)
     return LIB

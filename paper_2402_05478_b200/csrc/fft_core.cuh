@@ -118,16 +118,31 @@ template <int N> __device__ __forceinline__ int last_index(int i, int m, int q) 
 template <int N> __device__ __forceinline__ constexpr int first_reg(int m, int q) { return m * Plan<N>::radix(0) + q; }
 template <int N> __device__ __forceinline__ constexpr int last_reg(int m, int q) { return m * Plan<N>::radix(Plan<N>::NP - 1) + q; }
 
+// ---- shared-memory layouts of one exchange buffer ------------------------------------------------
+// Cols8 : [N][8] complex, element e of pencil p at e*8 + p.  With lane = (p, slot) any set of rows is
+//         conflict-free (each row is one full 128-byte wavefront), whatever the stride between rows.
+// Padded: one pencil per buffer, element e at e + (e >> 3) (one pad slot per 8 elements).  With lanes
+//         = consecutive slots of ONE pencil this keeps the stride-8 / stride-64 writes of the
+//         radix-8 passes on distinct 16-byte bank groups.
+struct Cols8 {
+    int p;
+    __device__ __forceinline__ int operator()(int e) const { return e * 8 + p; }
+};
+struct Padded {
+    __device__ __forceinline__ int operator()(int e) const { return e + (e >> 3); }
+    __host__ __device__ static constexpr int size(int n) { return n + (n >> 3) + 1; }
+};
+
 // ---- the passes ----------------------------------------------------------------------------
 // tw[j] = exp(-2*pi*i*j/N), j = 0..N-1 (forward); the inverse conjugates on the fly.
-// sm: this pencil group's [N][8] buffer.  i: slot in pencil (0..TP-1).  p: pencil (0..7).
-template <int N, bool INV, int S, int P>
+// sm + lay(e): where element e of this thread's pencil lives between passes.  i: slot (0..TP-1).
+template <int N, bool INV, int S, int P, typename L>
 struct Pass {
     static constexpr int R = Plan<N>::radix(S);
     static constexpr int E = Plan<N>::E;
     static constexpr int TP = Plan<N>::TP;
     static constexpr bool LAST = (S == Plan<N>::NP - 1);
-    __device__ __forceinline__ static void run(cplx (&v)[E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
+    __device__ __forceinline__ static void run(cplx (&v)[E], cplx* sm, int i, const L& lay, const cplx* __restrict__ tw) {
 #pragma unroll
         for (int m = 0; m < E / R; ++m) {
             const int b = i + TP * m;
@@ -144,7 +159,7 @@ struct Pass {
             if constexpr (!LAST) {
                 const int j = (b - k) * R + k;
 #pragma unroll
-                for (int q = 0; q < R; ++q) sm[(j + q * P) * 8 + p] = v[m * R + q];
+                for (int q = 0; q < R; ++q) sm[lay(j + q * P)] = v[m * R + q];
             }
         }
         if constexpr (!LAST) {
@@ -153,9 +168,9 @@ struct Pass {
 #pragma unroll
             for (int m = 0; m < E / Rn; ++m)
 #pragma unroll
-                for (int q = 0; q < Rn; ++q) v[m * Rn + q] = sm[(i + TP * m + q * (N / Rn)) * 8 + p];
+                for (int q = 0; q < Rn; ++q) v[m * Rn + q] = sm[lay(i + TP * m + q * (N / Rn))];
             __syncthreads();
-            Pass<N, INV, S + 1, P * R>::run(v, sm, i, p, tw);
+            Pass<N, INV, S + 1, P * R, L>::run(v, sm, i, lay, tw);
         }
     }
 };
@@ -164,7 +179,14 @@ struct Pass {
 // last-pass outputs (see last_index).  All threads of the CTA must call it (it synchronises).
 template <int N, bool INV>
 __device__ __forceinline__ void pencil_fft(cplx (&v)[Plan<N>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
-    Pass<N, INV, 0, 1>::run(v, sm, i, p, tw);
+    Cols8 lay{p};
+    Pass<N, INV, 0, 1, Cols8>::run(v, sm, i, lay, tw);
+}
+// same, one pencil per (padded) buffer
+template <int N, bool INV>
+__device__ __forceinline__ void pencil_fft_private(cplx (&v)[Plan<N>::E], cplx* sm, int i, const cplx* __restrict__ tw) {
+    Padded lay;
+    Pass<N, INV, 0, 1, Padded>::run(v, sm, i, lay, tw);
 }
 
 }  // namespace mhdfft

@@ -19,8 +19,8 @@ namespace {
 constexpr int kMaxShell = 2048;
 
 // kernel classes timed by mhd_profile_begin / mhd_profile_end, in hot-path order
-enum { K_Z_INV = 0, K_Y_INV, K_X_C2R, K_PRODUCTS, K_X_R2C, K_Y_FWD, K_Z_FWD, K_STAGE, K_NCLASS };
-const char* const kClassNames[K_NCLASS] = {"fft_z_inv", "fft_y_inv", "fft_x_c2r", "products", "fft_x_r2c", "fft_y_fwd", "fft_z_fwd", "stage"};
+enum { K_Z_INV = 0, K_Y_INV, K_X_C2R, K_PRODUCTS, K_X_R2C, K_XFUSED, K_Y_FWD, K_Z_FWD, K_STAGE, K_NCLASS };
+const char* const kClassNames[K_NCLASS] = {"fft_z_inv", "fft_y_inv", "fft_x_c2r", "products", "fft_x_r2c", "x_fused", "fft_y_fwd", "fft_z_fwd", "stage"};
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -101,6 +101,7 @@ struct mhd_ctx {
     cudaGraphExec_t graph;     // one steady-state step (AB2 non-first / RK4), replayed by mhd_step
     int graph_ready;
     long long graph_launches;  // kernels inside the captured step
+    int xfuse;                 // fused x pass available for this nx (and not disabled by MHD_NO_XFUSE)
     int profiling;             // mhd_profile_begin: eager steps with CUDA events around every kernel
     std::vector<cudaEvent_t>* prof_ev;   // [K_NCLASS] start/stop pairs
     char err[256];
@@ -143,8 +144,8 @@ SpecGeom spec_geom(const Geometry& g) {
     return s;
 }
 
-// compact spectral fields -> real fields  (z inverse, y inverse, x complex-to-real)
-cudaError_t inverse_fields(mhd_ctx* c, const double2* src, int nf, double* real_out) {
+// compact spectral fields -> W2 = [field][z][y][px] half-spectrum rows (z inverse, y inverse)
+cudaError_t inverse_zy(mhd_ctx* c, const double2* src, int nf) {
     const Geometry& g = c->g;
     cudaError_t e;
     const double2* ysrc = src;
@@ -166,11 +167,21 @@ cudaError_t inverse_fields(mhd_ctx* c, const double2* src, int nf, double* real_
         a.inner = g.px; a.nk_in = g.nky; a.nk_out = g.ny; a.scale = 1.0;
         if ((e = timed(c, K_Y_INV, [&] { return launch_fft_axis(g.ny, true, a, c->twy, c->st); })) != cudaSuccess) return e;
     }
+    return cudaSuccess;
+}
+
+// compact spectral fields -> real fields  (z inverse, y inverse, x complex-to-real)
+cudaError_t inverse_fields(mhd_ctx* c, const double2* src, int nf, double* real_out) {
+    const Geometry& g = c->g;
+    cudaError_t e;
+    if ((e = inverse_zy(c, src, nf)) != cudaSuccess) return e;
     RowArgs r;
     r.spec = c->W2; r.real = real_out; r.spec_pitch = g.px; r.real_pitch = g.nx;
     r.nrows = (long long)nf * g.nz * g.ny; r.nkx = g.nkx; r.scale = 1.0 / (double)g.npts;
     return timed(c, K_X_C2R, [&] { return launch_fft_rows(g.nx, true, r, c->twx, c->st); });
 }
+
+cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst);
 
 // real fields -> compact spectral fields (x real-to-complex, y forward, z forward), unnormalised
 cudaError_t forward_fields(mhd_ctx* c, const double* real_in, int nf, double2* dst) {
@@ -180,6 +191,13 @@ cudaError_t forward_fields(mhd_ctx* c, const double* real_in, int nf, double2* d
     r.spec = c->W2; r.real = const_cast<double*>(real_in); r.spec_pitch = g.px; r.real_pitch = g.nx;
     r.nrows = (long long)nf * g.nz * g.ny; r.nkx = g.nkx; r.scale = 1.0;
     if ((e = timed(c, K_X_R2C, [&] { return launch_fft_rows(g.nx, false, r, c->twx, c->st); })) != cudaSuccess) return e;
+    return forward_yz(c, nf, dst);
+}
+
+// W2 half-spectrum rows -> compact spectral fields (y forward, z forward)
+cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst) {
+    const Geometry& g = c->g;
+    cudaError_t e;
     {
         AxisArgs a;
         a.in = c->W2; a.out = (g.nz > 1) ? c->W1 : dst; a.nouter = (long long)nf * g.nz;
@@ -203,9 +221,18 @@ cudaError_t forward_fields(mhd_ctx* c, const double* real_in, int nf, double2* d
 cudaError_t rhs_stage(mhd_ctx* c, int mode) {
     const Geometry& g = c->g;
     cudaError_t e;
-    if ((e = inverse_fields(c, c->S, c->hydro ? 4 : NFIELD, c->Rf)) != cudaSuccess) return e;
-    if ((e = timed(c, K_PRODUCTS, [&] { return launch_products(c->Rf, c->Rg, g.npts, c->hydro, c->st); })) != cudaSuccess) return e;
-    if ((e = forward_fields(c, c->Rg, c->hydro ? 9 : NPROD, c->G)) != cudaSuccess) return e;
+    if (c->xfuse) {   // x inverse + products + x forward in one kernel, in place on W2
+        if ((e = inverse_zy(c, c->S, c->hydro ? 4 : NFIELD)) != cudaSuccess) return e;
+        XFusedArgs x;
+        x.w2 = c->W2; x.field_stride = g.w2field; x.nrows = (long long)g.nz * g.ny; x.px = g.px; x.nkx = g.nkx;
+        x.scale = 1.0 / (double)g.npts;
+        if ((e = timed(c, K_XFUSED, [&] { return launch_xfused(g.nx, x, c->hydro, c->twx, c->st); })) != cudaSuccess) return e;
+        if ((e = forward_yz(c, c->hydro ? 9 : NPROD, c->G)) != cudaSuccess) return e;
+    } else {
+        if ((e = inverse_fields(c, c->S, c->hydro ? 4 : NFIELD, c->Rf)) != cudaSuccess) return e;
+        if ((e = timed(c, K_PRODUCTS, [&] { return launch_products(c->Rf, c->Rg, g.npts, c->hydro, c->st); })) != cudaSuccess) return e;
+        if ((e = forward_fields(c, c->Rg, c->hydro ? 9 : NPROD, c->G)) != cudaSuccess) return e;
+    }
     StageArgs s;
     s.g = spec_geom(g); s.S = c->S; s.G = c->G; s.H = c->H; s.Acc = c->Acc;
     s.nu = c->nu; s.eta = c->eta; s.cs2 = c->cs * c->cs; s.dt = c->dt; s.mode = mode; s.hydro = c->hydro;
@@ -300,6 +327,7 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     c->g = g; c->nu = nu; c->eta = eta; c->cs = cs; c->dt = dt;
     c->integrator = integrator; c->flags = flags; c->hydro = (flags & MHD_FLAG_HYDRO) ? 1 : 0;
     c->st = (cudaStream_t)stream; c->ws = (char*)workspace; c->L = L;
+    c->xfuse = xfused_supported(nx) && getenv("MHD_NO_XFUSE") == nullptr;
     c->prof_ev = new (std::nothrow) std::vector<cudaEvent_t>[K_NCLASS];
     if (!c->prof_ev) { delete c; return MHD_ENOMEM; }
     c->twx = (double2*)(c->ws + L.twx); c->twy = (double2*)(c->ws + L.twy); c->twz = (double2*)(c->ws + L.twz);

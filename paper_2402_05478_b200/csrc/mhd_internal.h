@@ -30,6 +30,17 @@ bool fft_size_supported(int n);
 cudaError_t launch_fft_axis(int n, bool inverse, const AxisArgs& a, const double2* tw, cudaStream_t st);
 cudaError_t launch_fft_rows(int n, bool inverse, const RowArgs& a, const double2* tw, cudaStream_t st);
 
+// ---- fused x pass (xfused_kernel.cu): C2R-x -> products -> R2C-x, in place on [field][row][px] ----
+struct XFusedArgs {
+    double2* w2;              // inputs: fields 0..6 (0..3 hydro); outputs: product fields 0..11 (0..8 hydro)
+    long long field_stride;   // complex elements per field
+    long long nrows;          // nz*ny
+    int px, nkx;              // row pitch and stored modes per row
+    double scale;             // 1/(nx*ny*nz), applied to the inverse transforms
+};
+bool xfused_supported(int n);
+cudaError_t launch_xfused(int n, const XFusedArgs& a, int hydro, const double2* tw, cudaStream_t st);
+
 // ---- pointwise / spectral kernels (mhd_kernels.cu) ------------------------------------------
 // real-space field order in a block of consecutive arrays (stride = points per field)
 enum { F_RHO = 0, F_MX, F_MY, F_MZ, F_BX, F_BY, F_BZ, NFIELD = 7 };
