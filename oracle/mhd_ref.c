@@ -218,6 +218,8 @@ struct mhd_ref_ctx {
     double* g[NPROD];       /* real-space products                     */
     cplx* G[NPROD];         /* their transforms                        */
     cplx* tmp;              /* scratch half-spectrum (c2r3 destroys its input) */
+    double kfac[3];         /* 2*pi/L_i: physical wavenumber = kfac[i] * integer index (1.0 on the 2*pi box) */
+    cplx* Fh[3];            /* masked transform of the steady body force f of eq. (2), or NULL */
     int have_fields, have_history;
     long long step;
     double time;
@@ -237,6 +239,7 @@ static void free_ctx(mhd_ref_ctx* c) {
     for (int i = 0; i < NFIELD; ++i) { free(c->S[i]); free(c->R[i]); free(c->Rold[i]); free(c->S0[i]); free(c->Acc[i]); free(c->f[i]); }
     for (int i = 0; i < NPROD; ++i) { free(c->g[i]); free(c->G[i]); }
     free(c->tmp);
+    for (int i = 0; i < 3; ++i) free(c->Fh[i]);
     plan3_free(&c->plan);
     free(c);
 }
@@ -254,6 +257,7 @@ int mhd_ref_create(mhd_ref_ctx** out, int nx, int ny, int nz, double nu, double 
     c->nu = nu; c->eta = eta; c->cs = cs; c->dt = dt;
     c->integrator = integrator; c->flags = flags;
     c->nr = (size_t)nx * ny * nz; c->nc = (size_t)c->nxh * ny * nz;
+    c->kfac[0] = c->kfac[1] = c->kfac[2] = 1.0;
     if (plan3_init(&c->plan, nx, ny, nz)) { free_ctx(c); return MHD_REF_ENOMEM; }
     int ok = 1;
     for (int i = 0; i < NFIELD; ++i) {
@@ -296,6 +300,34 @@ static void apply_mask(const mhd_ref_ctx* c, cplx* a) {
             for (int jx = 0; jx < c->nxh; ++jx)
                 if (!mask_keep(c, jx, wavenumber(jy, c->ny), wavenumber(jz, c->nz)))
                     a[((size_t)jz * c->ny + jy) * c->nxh + jx] = 0.0;
+}
+
+/* box lengths: k_i = (2*pi/L_i) n_i   (PAPER.md:161 uses Lx = 1, Ly = 2; every other test the 2*pi box) */
+int mhd_ref_set_box(mhd_ref_ctx* c, double lx, double ly, double lz) {
+    if (!c || !(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0) || !isfinite(lx) || !isfinite(ly) || !isfinite(lz)) return MHD_REF_EINVAL;
+    const double two_pi = 6.283185307179586476925286766559;
+    const double l[3] = {lx, ly, lz};
+    for (int i = 0; i < 3; ++i) c->kfac[i] = (l[i] == two_pi) ? 1.0 : two_pi / l[i];
+    return MHD_REF_OK;
+}
+
+/* steady body force f of eq. (2): stored as its masked transform */
+int mhd_ref_set_forcing(mhd_ref_ctx* c, const double* fx, const double* fy, const double* fz) {
+    if (!c) return MHD_REF_EINVAL;
+    const double* f[3] = {fx, fy, fz};
+    if (!fx && !fy && !fz) {
+        for (int i = 0; i < 3; ++i) { free(c->Fh[i]); c->Fh[i] = NULL; }
+        return MHD_REF_OK;
+    }
+    if (!fx || !fy || !fz) return MHD_REF_EINVAL;
+    for (int i = 0; i < 3; ++i) {
+        if (!c->Fh[i]) c->Fh[i] = (cplx*)calloc(c->nc, sizeof(cplx));
+        if (!c->Fh[i]) return MHD_REF_ENOMEM;
+        memcpy(c->g[0], f[i], sizeof(double) * c->nr);
+        r2c3(&c->plan, c->g[0], c->Fh[i]);
+        apply_mask(c, c->Fh[i]);
+    }
+    return MHD_REF_OK;
 }
 
 /* step 1 of SURVEY.md §8(c.2): m = rho*u; forward-FFT the 7 fields; mask; reset history */
@@ -371,9 +403,10 @@ static void rhs(mhd_ref_ctx* c, cplx* const* S, cplx* const* R) {
         for (int jy = 0; jy < c->ny; ++jy)
             for (int jx = 0; jx < c->nxh; ++jx) {
                 size_t q = ((size_t)jz * c->ny + jy) * c->nxh + jx;
-                double kx = jx, ky = wavenumber(jy, c->ny), kz = wavenumber(jz, c->nz);
+                int ny_ = wavenumber(jy, c->ny), nz_ = wavenumber(jz, c->nz);
+                double kx = c->kfac[0] * jx, ky = c->kfac[1] * ny_, kz = c->kfac[2] * nz_;
                 double k2 = kx * kx + ky * ky + kz * kz;
-                double M = mask_keep(c, jx, (int)ky, (int)kz) ? 1.0 : 0.0;
+                double M = mask_keep(c, jx, ny_, nz_) ? 1.0 : 0.0;
                 /* eq. (1): d rho/dt = -div m */
                 R[F_RHO][q] = -I * (kx * S[F_MX][q] + ky * S[F_MY][q] + kz * S[F_MZ][q]);
                 /* eq. (2)+(3): d m_i/dt = -d_j T_ij - cs^2 d_i rho + nu lap u_i */
@@ -383,6 +416,8 @@ static void rhs(mhd_ref_ctx* c, cplx* const* S, cplx* const* R) {
                                   - I * ky * cs2 * S[F_RHO][q] - nu * k2 * G[P_UY][q]);
                 R[F_MZ][q] = M * (-I * (kx * G[P_TXZ][q] + ky * G[P_TYZ][q] + kz * G[P_TZZ][q])
                                   - I * kz * cs2 * S[F_RHO][q] - nu * k2 * G[P_UZ][q]);
+                /* eq. (2): + f (steady body force; Fh is already masked) */
+                if (c->Fh[0]) { R[F_MX][q] += c->Fh[0][q]; R[F_MY][q] += c->Fh[1][q]; R[F_MZ][q] += c->Fh[2][q]; }
                 /* eq. (4): d B/dt = curl (u x B) + eta lap B */
                 if (hydro) {
                     R[F_BX][q] = 0.0; R[F_BY][q] = 0.0; R[F_BZ][q] = 0.0;
@@ -524,7 +559,7 @@ int mhd_ref_diagnostics(mhd_ref_ctx* c, mhd_ref_diag* d, double* ekin_spec, doub
         for (int jy = 0; jy < c->ny; ++jy)
             for (int jx = 0; jx < c->nxh; ++jx) {
                 size_t q = ((size_t)jz * c->ny + jy) * c->nxh + jx;
-                double kx = jx, ky = wavenumber(jy, c->ny), kz = wavenumber(jz, c->nz);
+                double kx = c->kfac[0] * jx, ky = c->kfac[1] * wavenumber(jy, c->ny), kz = c->kfac[2] * wavenumber(jz, c->nz);
                 c->tmp[q] = I * (kx * c->S[F_BX][q] + ky * c->S[F_BY][q] + kz * c->S[F_BZ][q]);
             }
     c2r3(&c->plan, c->tmp, c->g[0]);
@@ -532,16 +567,46 @@ int mhd_ref_diagnostics(mhd_ref_ctx* c, mhd_ref_diag* d, double* ekin_spec, doub
     for (size_t p = 0; p < c->nr; ++p) { double a = fabs(c->g[0][p]); if (a > mx) mx = a; if (!isfinite(a)) bad = 1; }
     d->max_divb = mx;
 
+    /* u^ = FFT(m/rho) over EVERY mode (u is not band-limited): needed by the paper diagnostics and the spectra */
+    to_real(c, c->S);
+    for (int i = 0; i < 3; ++i) {
+        for (size_t p = 0; p < c->nr; ++p) c->g[i][p] = c->f[F_MX + i][p] / c->f[F_RHO][p];
+        r2c3(&c->plan, c->g[i], c->G[i]);
+    }
+    /* Omega(t) = <|curl u|^2>, <|curl B|^2>, <|u|^2>, Rayleigh quotient eq. (14), as
+     * sums over the full spectrum (Parseval): half-spectrum entries with 0 < kx < nx/2 stand for two modes. */
+    {
+        ksum en = {0, 0}, cu = {0, 0}, u2 = {0, 0};
+        for (int jz = 0; jz < c->nz; ++jz)
+            for (int jy = 0; jy < c->ny; ++jy)
+                for (int jx = 0; jx < c->nxh; ++jx) {
+                    size_t q = ((size_t)jz * c->ny + jy) * c->nxh + jx;
+                    double kx = c->kfac[0] * jx, ky = c->kfac[1] * wavenumber(jy, c->ny), kz = c->kfac[2] * wavenumber(jz, c->nz);
+                    double w = (jx == 0 || 2 * jx == c->nx) ? 1.0 : 2.0;
+                    cplx ux = c->G[0][q], uy = c->G[1][q], uz = c->G[2][q];
+                    cplx wx = ky * uz - kz * uy, wy = kz * ux - kx * uz, wz = kx * uy - ky * ux;      /* (k x u^) */
+                    ksum_add(&en, w * (creal(wx) * creal(wx) + cimag(wx) * cimag(wx) + creal(wy) * creal(wy) + cimag(wy) * cimag(wy) +
+                                       creal(wz) * creal(wz) + cimag(wz) * cimag(wz)));
+                    ksum_add(&u2, w * (creal(ux) * creal(ux) + cimag(ux) * cimag(ux) + creal(uy) * creal(uy) + cimag(uy) * cimag(uy) +
+                                       creal(uz) * creal(uz) + cimag(uz) * cimag(uz)));
+                    cplx bx = c->S[F_BX][q], by = c->S[F_BY][q], bz = c->S[F_BZ][q];
+                    cplx jx_ = ky * bz - kz * by, jy_ = kz * bx - kx * bz, jz_ = kx * by - ky * bx;   /* (k x B^) */
+                    ksum_add(&cu, w * (creal(jx_) * creal(jx_) + cimag(jx_) * cimag(jx_) + creal(jy_) * creal(jy_) + cimag(jy_) * cimag(jy_) +
+                                       creal(jz_) * creal(jz_) + cimag(jz_) * cimag(jz_)));
+                }
+        d->enstrophy = ksum_get(&en) * Ninv * Ninv;
+        d->current2 = ksum_get(&cu) * Ninv * Ninv;
+        d->u2 = ksum_get(&u2) * Ninv * Ninv;
+        double den = d->u2 + d->emag;                 /* <|u|^2> + 1/2 <|B|^2>,  emag = 1/2 <|B|^2> */
+        d->rayleigh_q = den > 0.0 ? (d->enstrophy + 0.5 * d->current2) / den : 0.0;
+    }
+
     /* shell spectra: s = round(|k|); velocity power 1/2|u^|^2/N^2 (u = m/rho, not density weighted),
      * magnetic power 1/2|B^|^2/N^2; half-spectrum entries with 0 < kx < nx/2 stand for two modes. */
     if (nshell > 0) {
+        if (c->kfac[0] != 1.0 || c->kfac[1] != 1.0 || (c->nz > 1 && c->kfac[2] != 1.0)) return MHD_REF_EINVAL;   /* 2*pi box only */
         ksum* ks = (ksum*)calloc((size_t)nshell * 2, sizeof(ksum));
         if (!ks) return MHD_REF_ENOMEM;
-        to_real(c, c->S);
-        for (int i = 0; i < 3; ++i) {
-            for (size_t p = 0; p < c->nr; ++p) c->g[i][p] = c->f[F_MX + i][p] / c->f[F_RHO][p];
-            r2c3(&c->plan, c->g[i], c->G[i]);
-        }
         for (int jz = 0; jz < c->nz; ++jz)
             for (int jy = 0; jy < c->ny; ++jy)
                 for (int jx = 0; jx < c->nxh; ++jx) {

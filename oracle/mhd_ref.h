@@ -13,7 +13,9 @@
  * Parity pins (tests/test_oracle_*.py): brute-force DFT, numpy.fft, exact single-mode viscous /
  * resistive decay, circularly polarised Alfven wave (sign of eq. 4), sound / fast-wave frequency,
  * exact invariants, div B at roundoff, ideal-limit energy drift order, energy balance, cyclic
- * axis permutation, KH linear growth.  PARITY UNPINNED by the paper (API definitions fixed by
+ * axis permutation, KH linear growth; box lengths by the exact rescaling x -> 2*pi*x/L of the
+ * equations; forcing by the exact forced shear-wave recurrence and the momentum budget; enstrophy /
+ * Rayleigh quotient by Beltrami (curl u = k0 u) closed forms and a numpy restatement.  PARITY UNPINNED by the paper (API definitions fixed by
  * SURVEY.md §8(c.3), not by PAPER.md): the order of the Adams-Bashforth scheme (AB2 with an Euler
  * first step), the sound speed of each config, and the definition of the shell spectra.
  *
@@ -36,6 +38,12 @@ enum { MHD_REF_FLAG_HYDRO = 1u, MHD_REF_FLAG_NO_DEALIAS = 2u };
 typedef struct {
     long long step;
     double time, ekin, emag, eiso, mass, mom[3], bmean[3], max_divb;
+    /* paper diagnostics, all from the spectra of u = m/rho (every mode) and B:
+     *   enstrophy  = <|curl u|^2> = sum_k |k x u^(k)|^2 / N^2      Omega(t)
+     *   current2   = <|curl B|^2> = sum_k |k x B^(k)|^2 / N^2
+     *   u2         = <|u|^2>      = sum_k |u^(k)|^2 / N^2
+     *   rayleigh_q = (enstrophy + current2/2) / (u2 + <|B|^2>/2)     eq. (14) */
+    double enstrophy, current2, u2, rayleigh_q;
 } mhd_ref_diag;
 
 /* threads used by the row loops (OpenMP); results do not depend on it */
@@ -51,6 +59,13 @@ int mhd_ref_fft_c2r(int nx, int ny, int nz, int batch, const double* in_complex,
 int  mhd_ref_create(mhd_ref_ctx** out, int nx, int ny, int nz, double nu, double eta, double cs, double dt,
                     int integrator, unsigned flags);
 void mhd_ref_destroy(mhd_ref_ctx*);
+/* Box lengths (the KH test uses Lx = 1, Ly = 2): wavenumbers become k_i = 2*pi*n_i/L_i.
+ * Default 2*pi per axis (k = n exactly).  The 2/3 mask stays a test on the integer n_i.  lz is ignored
+ * when nz == 1.  Shell spectra are defined for the 2*pi box only. */
+int  mhd_ref_set_box(mhd_ref_ctx*, double lx, double ly, double lz);
+/* Steady body force f(x) of eq. (2) ("+ f"; App. B eqs B2-B3): its masked
+ * transform is added to the momentum right-hand side.  NULL, NULL, NULL switches it off. */
+int  mhd_ref_set_forcing(mhd_ref_ctx*, const double* fx, const double* fy, const double* fz);
 int  mhd_ref_set_fields(mhd_ref_ctx*, const double* rho, const double* ux, const double* uy, const double* uz,
                         const double* bx, const double* by, const double* bz);
 int  mhd_ref_step(mhd_ref_ctx*, int nsteps);

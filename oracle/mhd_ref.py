@@ -36,7 +36,8 @@ def build(force: bool = False) -> str:
 class Diag(C.Structure):
     _fields_ = [("step", C.c_longlong), ("time", C.c_double), ("ekin", C.c_double), ("emag", C.c_double),
                 ("eiso", C.c_double), ("mass", C.c_double), ("mom", C.c_double * 3),
-                ("bmean", C.c_double * 3), ("max_divb", C.c_double)]
+                ("bmean", C.c_double * 3), ("max_divb", C.c_double),
+                ("enstrophy", C.c_double), ("current2", C.c_double), ("u2", C.c_double), ("rayleigh_q", C.c_double)]
 
 
 _lib = None
@@ -57,6 +58,8 @@ def lib():
         L.mhd_ref_destroy.argtypes = [C.c_void_p]
         L.mhd_ref_destroy.restype = None
         L.mhd_ref_set_fields.argtypes = [C.c_void_p] + [_dp] * 7
+        L.mhd_ref_set_box.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
+        L.mhd_ref_set_forcing.argtypes = [C.c_void_p] + [_dp] * 3
         L.mhd_ref_get_fields.argtypes = [C.c_void_p] + [_dp] * 7
         L.mhd_ref_step.argtypes = [C.c_void_p, C.c_int]
         L.mhd_ref_diagnostics.argtypes = [C.c_void_p, C.POINTER(Diag), _dp, _dp, C.c_int]
@@ -152,6 +155,19 @@ class RefSolver:
         if rc != OK:
             raise RuntimeError(f"mhd_ref_set_fields: {rc}")
 
+    def set_box(self, lx, ly, lz):
+        rc = lib().mhd_ref_set_box(self._h, float(lx), float(ly), float(lz))
+        if rc != OK:
+            raise ValueError(f"mhd_ref_set_box: {rc}")
+
+    def set_forcing(self, fx=None, fy=None, fz=None):
+        arrs = [None if a is None else _f64(a) for a in (fx, fy, fz)]
+        for a in arrs:
+            assert a is None or a.shape == self.shape
+        rc = lib().mhd_ref_set_forcing(self._h, *[_p(a) for a in arrs])
+        if rc != OK:
+            raise ValueError(f"mhd_ref_set_forcing: {rc}")
+
     def step(self, n=1):
         rc = lib().mhd_ref_step(self._h, int(n))
         if rc != OK:
@@ -172,7 +188,8 @@ class RefSolver:
         if rc not in (OK, ENONFINITE):
             raise RuntimeError(f"mhd_ref_diagnostics: {rc}")
         out = dict(step=d.step, time=d.time, ekin=d.ekin, emag=d.emag, eiso=d.eiso, mass=d.mass,
-                   mom=np.array(d.mom[:]), bmean=np.array(d.bmean[:]), max_divb=d.max_divb, rc=rc)
+                   mom=np.array(d.mom[:]), bmean=np.array(d.bmean[:]), max_divb=d.max_divb, rc=rc,
+                   enstrophy=d.enstrophy, current2=d.current2, u2=d.u2, rayleigh_q=d.rayleigh_q)
         if nshell > 0:
             out["ekin_spec"] = ek[:nshell].copy()
             out["emag_spec"] = em[:nshell].copy()

@@ -33,6 +33,11 @@
 #define MHD_XF_PREFETCH 1
 #endif
 // threads per persistent CTA for N >= 256 (a multiple of 128): 384 = 6 rows in flight per SM at N = 512
+// twiddles w^2..w^7 of a radix-8 pass by multiplication from w: 0 = never (7 table reads), 1 = last pass, 2 = every pass.
+// The kernel is bound by shared-memory wavefronts (80 % of the LSU data pipe), not FP64 (43 %): 2 is fastest (B200, 512^3).
+#ifndef MHD_XF_TWCHAIN
+#define MHD_XF_TWCHAIN 2
+#endif
 #ifndef MHD_XF_THREADS
 #define MHD_XF_THREADS 384
 #endif
@@ -83,11 +88,24 @@ struct XPass {
             const int k = b & (P - 1);
             if constexpr (S > 0) {
                 const cplx* __restrict__ t = stw + XCfg<N>::tw_offset(S) + k;
+                if constexpr (R == 8 && (MHD_XF_TWCHAIN >= 2 || (MHD_XF_TWCHAIN == 1 && P >= 32))) {
+                    // the kernel is bound by shared-memory wavefronts, not FP64: read w and form w^2..w^7 by
+                    // multiplication (depth <= 3, a few ulp) instead of 7 conflict-free but 4-wavefront reads
+                    cplx w1 = t[0];
+                    if (INV) w1.y = -w1.y;
+                    const cplx w2 = cmul(w1, w1), w3 = cmul(w2, w1), w4 = cmul(w2, w2);
+                    const cplx w5 = cmul(w4, w1), w6 = cmul(w3, w3), w7 = cmul(w4, w3);
+                    v[m * R + 1] = cmul(v[m * R + 1], w1); v[m * R + 2] = cmul(v[m * R + 2], w2);
+                    v[m * R + 3] = cmul(v[m * R + 3], w3); v[m * R + 4] = cmul(v[m * R + 4], w4);
+                    v[m * R + 5] = cmul(v[m * R + 5], w5); v[m * R + 6] = cmul(v[m * R + 6], w6);
+                    v[m * R + 7] = cmul(v[m * R + 7], w7);
+                } else {
 #pragma unroll
-                for (int q = 1; q < R; ++q) {
-                    cplx w = t[(q - 1) * P];
-                    if (INV) w.y = -w.y;
-                    v[m * R + q] = cmul(v[m * R + q], w);
+                    for (int q = 1; q < R; ++q) {
+                        cplx w = t[(q - 1) * P];
+                        if (INV) w.y = -w.y;
+                        v[m * R + q] = cmul(v[m * R + q], w);
+                    }
                 }
             }
             bfly<R, INV>(&v[m * R]);
@@ -370,7 +388,7 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
                 for (int q = 0; q < RL; ++q) {
                     const int t = m + q * (E / RL);            // index i + TP*t
                     if (PRUNED && t < 5) continue;                   // N - k > N - nkx >= 5*TP
-                    if (t >= 1 && (TP * (t + 1) > N - nkx)) bufA[xpad(i + TP * t)] = v[m * RL + q];   // index range [TP*t, TP*t+TP) meets [N-nkx+1, N)
+                    if (t >= 1 && (TP * (t + 1) > N - nkx)) bufA[N - (i + TP * t)] = v[m * RL + q];   // index range [TP*t, TP*t+TP) meets [N-nkx+1, N)
                 }
             team_sync<TP>(team);
             if (ok) {
@@ -384,7 +402,7 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
                         const int k = i + TP * t;
                         if (t <= (PRUNED ? 2 : E / 2) && k < nkx) {
                             const cplx zk = v[m * RL + q];
-                            const cplx zm = (k == 0) ? zk : bufA[xpad(N - k)];
+                            const cplx zm = (k == 0) ? zk : bufA[k];      // Z[N-k], published at position N - index (unpadded: conflict-free both ways)
                             oa[k] = make_double2(0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y));
                             if (idb >= 0) ob[k] = make_double2(0.5 * (zk.y + zm.y), 0.5 * (zm.x - zk.x));
                         }
