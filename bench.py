@@ -273,7 +273,7 @@ def run_gpu(args):
     roofline = {"bound": "hbm", "kernel": top["kernel"], "achieved": top["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": top["frac"], "traffic": top["traffic"], "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": abytes[top["kernel"]]}
-    own_bytes = sum(abytes.values())
+    own_bytes = sum(k["algorithmic_gb"] * 1e9 * k["launches_per_step"] for k in kernels)   # only the kernel classes that ran
     step_roofline = {
         "design_bytes_per_step": own_bytes, "design_gbs": own_bytes / 1e9 / (ms_step * 1e-3),
         "design_frac_of_measured_peak": own_bytes / 1e9 / (ms_step * 1e-3) / peak,

@@ -43,7 +43,8 @@ enum { MHD_OK = 0, MHD_EINVAL = -1, MHD_ENOMEM = -2, MHD_ECUDA = -3, MHD_ESTATE 
 enum { MHD_AB2 = 0, MHD_RK4 = 1 };
 enum {
     MHD_FLAG_HYDRO = 1u,      /* B == 0 held exactly: induction and Lorentz terms skipped */
-    MHD_FLAG_NO_DEALIAS = 2u  /* keep every mode (tests only) */
+    MHD_FLAG_NO_DEALIAS = 2u, /* keep every mode (tests only) */
+    MHD_FLAG_FORCING = 4u     /* reserve workspace for the steady body force f of eq. (2) (mhd_set_forcing) */
 };
 
 /* mean values are volume averages <.> = (1/N) sum over the grid */
@@ -57,6 +58,11 @@ typedef struct {
     double mom[3];     /* <rho u> */
     double bmean[3];   /* <B> */
     double max_divb;   /* max_x |IFFT(i k . B^)| */
+    /* the paper's diagnostics, as sums over the spectra of u = m/rho (every mode, not only the retained ones) and B: */
+    double enstrophy;  /* <|curl u|^2> = sum_k |k x u^|^2 / N^2: mean-square vorticity Omega(t) */
+    double current2;   /* <|curl B|^2> = sum_k |k x B^|^2 / N^2 */
+    double u2;         /* <|u|^2> */
+    double rayleigh_q; /* (enstrophy + current2/2) / (u2 + <|B|^2>/2): Rayleigh quotient Q(t), eq. (14) */
 } mhd_diag;
 
 /* Bytes of device workspace mhd_create needs for this configuration (0 if the size is unsupported). */
@@ -70,6 +76,19 @@ size_t mhd_workspace_bytes(int nx, int ny, int nz, int integrator, unsigned flag
 int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, double cs, double dt,
                int integrator, unsigned flags, void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 void mhd_destroy(mhd_ctx* ctx);
+
+/* Box lengths (the KH test uses Lx = 1, Ly = 2; every other test the 2*pi box): wavenumbers become
+ * k_i = 2*pi*n_i/L_i.  Default 2*pi per axis (k = n exactly).  The 2/3 mask stays a test on the integers n_i; lz is
+ * ignored when nz == 1.  May be called at any time; takes effect from the next mhd_step / mhd_diagnostics.
+ * MHD_EINVAL unless every length is finite and > 0. */
+int mhd_set_box(mhd_ctx* ctx, double lx, double ly, double lz);
+
+/* Steady body force f(x) of eq. (2) ("+ f"; App. B eqs B2-B3), nx*ny*nz doubles per
+ * component on the grid (DEVICE pointers; the _host variant takes HOST pointers).  Its 2/3-masked transform is kept
+ * in the workspace and added to the momentum right-hand side of every later step.  NULL, NULL, NULL switches it off.
+ * Needs MHD_FLAG_FORCING at mhd_create (MHD_ESTATE otherwise).  Asynchronous; inputs are read, never written. */
+int mhd_set_forcing(mhd_ctx* ctx, const double* fx_dev, const double* fy_dev, const double* fz_dev);
+int mhd_set_forcing_host(mhd_ctx* ctx, const double* fx_host, const double* fy_host, const double* fz_host);
 
 /* Set the state from grid fields: m = rho*u, forward transform, 2/3 mask.
  * Resets step count, time and integrator history.  b* may be NULL with MHD_FLAG_HYDRO.
@@ -95,6 +114,7 @@ int mhd_get_fields_host(mhd_ctx* ctx, double* rho_host, double* ux_host, double*
  * Spectra (optional, nshell may be 0): shell s = round(|k|), s = 0..nshell-1,
  *   ekin_spec[s] = sum_{k in s} 1/2 |u^(k)|^2 / N^2   with u = m/rho (sums to 1/2 <|u|^2>),
  *   emag_spec[s] = sum_{k in s} 1/2 |B^(k)|^2 / N^2   (sums to emag).
+ * Spectra are defined on the 2*pi box only (MHD_EINVAL with nshell > 0 after mhd_set_box to another length).
  * Returns MHD_ENONFINITE (values still filled) if a NaN/Inf or rho <= 0 was seen, MHD_ECUDA on a
  * sticky CUDA error. */
 int mhd_diagnostics(mhd_ctx* ctx, mhd_diag* out_host, double* ekin_spec_host, double* emag_spec_host, int nshell);

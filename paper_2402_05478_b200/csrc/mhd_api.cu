@@ -51,10 +51,10 @@ bool make_geometry(int nx, int ny, int nz, unsigned flags, Geometry* g) {
 }
 
 struct Layout {
-    size_t twx, twy, twz, S, H, Acc, G, W1, W2, Rf, Rg, red, total;
+    size_t twx, twy, twz, S, H, Acc, Fh, G, W1, W2, Rf, Rg, red, total;
 };
 
-Layout make_layout(const Geometry& g, int integrator) {
+Layout make_layout(const Geometry& g, int integrator, unsigned flags) {
     Layout L;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
@@ -64,6 +64,7 @@ Layout make_layout(const Geometry& g, int integrator) {
     L.S = take(sizeof(double2) * g.fieldc * NFIELD);
     L.H = take(sizeof(double2) * g.fieldc * NFIELD);
     L.Acc = take(integrator == MHD_RK4 ? sizeof(double2) * g.fieldc * NFIELD : 0);
+    L.Fh = take((flags & MHD_FLAG_FORCING) ? sizeof(double2) * g.fieldc * 3 : 0);
     L.G = take(sizeof(double2) * g.fieldc * NPROD);
     L.W1 = take(g.nz > 1 ? sizeof(double2) * g.w1field * NPROD : 0);
     L.W2 = take(sizeof(double2) * g.w2field * NPROD);
@@ -94,7 +95,9 @@ struct mhd_ctx {
     cudaStream_t st;
     char* ws;
     Layout L;
-    double2 *twx, *twy, *twz, *S, *H, *Acc, *G, *W1, *W2;
+    double2 *twx, *twy, *twz, *S, *H, *Acc, *Fh, *G, *W1, *W2;
+    double kf[3];              // 2*pi/L per axis (1.0 on the 2*pi box)
+    int have_forcing;          // Fh holds a force (mhd_set_forcing)
     double *Rf, *Rg, *red_partial, *red_result, *spec_dev;
     long long step;
     int have_fields, have_history;
@@ -236,6 +239,7 @@ cudaError_t rhs_stage(mhd_ctx* c, int mode) {
     StageArgs s;
     s.g = spec_geom(g); s.S = c->S; s.G = c->G; s.H = c->H; s.Acc = c->Acc;
     s.nu = c->nu; s.eta = c->eta; s.cs2 = c->cs * c->cs; s.dt = c->dt; s.mode = mode; s.hydro = c->hydro;
+    s.F = c->have_forcing ? c->Fh : nullptr; s.kfx = c->kf[0]; s.kfy = c->kf[1]; s.kfz = c->kf[2];
     return timed(c, K_STAGE, [&] { return launch_stage(s, c->st); });
 }
 
@@ -306,7 +310,7 @@ size_t mhd_workspace_bytes(int nx, int ny, int nz, int integrator, unsigned flag
     Geometry g;
     if (!make_geometry(nx, ny, nz, flags, &g)) return 0;
     if (integrator != MHD_AB2 && integrator != MHD_RK4) return 0;
-    return make_layout(g, integrator).total;
+    return make_layout(g, integrator, flags).total;
 }
 
 int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, double cs, double dt,
@@ -318,8 +322,8 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     if (integrator != MHD_AB2 && integrator != MHD_RK4) return MHD_EINVAL;
     if (!(nu >= 0.0) || !(eta >= 0.0) || !(cs >= 0.0) || !(dt > 0.0)) return MHD_EINVAL;
     if (!isfinite(nu) || !isfinite(eta) || !isfinite(cs) || !isfinite(dt)) return MHD_EINVAL;
-    if (flags & ~(MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS)) return MHD_EINVAL;
-    const Layout L = make_layout(g, integrator);
+    if (flags & ~(MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS | MHD_FLAG_FORCING)) return MHD_EINVAL;
+    const Layout L = make_layout(g, integrator, flags);
     if (!workspace || workspace_bytes < L.total || ((size_t)workspace & 255u)) return MHD_EINVAL;
     mhd_ctx* c = new (std::nothrow) mhd_ctx();
     if (!c) return MHD_ENOMEM;
@@ -332,6 +336,7 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     if (!c->prof_ev) { delete c; return MHD_ENOMEM; }
     c->twx = (double2*)(c->ws + L.twx); c->twy = (double2*)(c->ws + L.twy); c->twz = (double2*)(c->ws + L.twz);
     c->S = (double2*)(c->ws + L.S); c->H = (double2*)(c->ws + L.H); c->Acc = (double2*)(c->ws + L.Acc);
+    c->Fh = (double2*)(c->ws + L.Fh); c->kf[0] = c->kf[1] = c->kf[2] = 1.0;
     c->G = (double2*)(c->ws + L.G); c->W1 = (double2*)(c->ws + L.W1); c->W2 = (double2*)(c->ws + L.W2);
     c->Rf = (double*)(c->ws + L.Rf); c->Rg = (double*)(c->ws + L.Rg);
     c->red_partial = (double*)(c->ws + L.red);
@@ -360,6 +365,50 @@ void mhd_destroy(mhd_ctx* c) {
         delete[] c->prof_ev;
     }
     delete c;
+}
+
+// the captured step bakes in the stage kernel's arguments: drop it when they change
+static void invalidate_graph(mhd_ctx* c) {
+    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
+    c->graph_ready = 0;
+}
+
+int mhd_set_box(mhd_ctx* c, double lx, double ly, double lz) {
+    if (!c) return MHD_EINVAL;
+    if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0) || !isfinite(lx) || !isfinite(ly) || !isfinite(lz))
+        return fail(c, MHD_EINVAL, "mhd_set_box: lengths must be finite and > 0");
+    const double two_pi = 6.283185307179586476925286766559;
+    const double l[3] = {lx, ly, lz};
+    for (int i = 0; i < 3; ++i) c->kf[i] = (l[i] == two_pi) ? 1.0 : two_pi / l[i];
+    invalidate_graph(c);
+    return MHD_OK;
+}
+
+int mhd_set_forcing(mhd_ctx* c, const double* fx, const double* fy, const double* fz) {
+    if (!c) return MHD_EINVAL;
+    if (!fx && !fy && !fz) { c->have_forcing = 0; invalidate_graph(c); return MHD_OK; }
+    if (!fx || !fy || !fz) return fail(c, MHD_EINVAL, "mhd_set_forcing: give all three components or none");
+    if (!(c->flags & MHD_FLAG_FORCING)) return fail(c, MHD_ESTATE, "mhd_set_forcing: context created without MHD_FLAG_FORCING");
+    const long long n = c->g.npts;
+    const size_t fb = sizeof(double) * n;
+    const double* f[3] = {fx, fy, fz};
+    for (int i = 0; i < 3; ++i)
+        if (f[i] != c->Rg + i * n) CK(cudaMemcpyAsync(c->Rg + i * n, f[i], fb, cudaMemcpyDeviceToDevice, c->st));
+    CK(forward_fields(c, c->Rg, 3, c->Fh));
+    c->have_forcing = 1;
+    invalidate_graph(c);
+    return MHD_OK;
+}
+
+int mhd_set_forcing_host(mhd_ctx* c, const double* fx, const double* fy, const double* fz) {
+    if (!c) return MHD_EINVAL;
+    if (!fx && !fy && !fz) return mhd_set_forcing(c, nullptr, nullptr, nullptr);
+    if (!fx || !fy || !fz) return fail(c, MHD_EINVAL, "mhd_set_forcing_host: give all three components or none");
+    if (!(c->flags & MHD_FLAG_FORCING)) return fail(c, MHD_ESTATE, "mhd_set_forcing_host: context created without MHD_FLAG_FORCING");
+    const long long n = c->g.npts;
+    const double* f[3] = {fx, fy, fz};
+    for (int i = 0; i < 3; ++i) CK(cudaMemcpyAsync(c->Rg + i * n, f[i], sizeof(double) * n, cudaMemcpyHostToDevice, c->st));
+    return mhd_set_forcing(c, c->Rg, c->Rg + n, c->Rg + 2 * n);
 }
 
 int mhd_set_fields(mhd_ctx* c, const double* rho, const double* ux, const double* uy, const double* uz,
@@ -490,8 +539,10 @@ int mhd_diagnostics(mhd_ctx* c, mhd_diag* out, double* ekin_spec, double* emag_s
     const SpecGeom sg = spec_geom(g);
     CK(inverse_fields(c, c->S, c->hydro ? 4 : NFIELD, c->Rf));
     CK(launch_reduce_fields(c->Rf, n, c->hydro, c->red_partial, c->red_result, c->st));
-    if (nshell > 0) {
-        // Velocity spectrum: u = m/rho is not band-limited, and the spectrum is defined over ALL modes
+    if (nshell > 0 && (c->kf[0] != 1.0 || c->kf[1] != 1.0 || (g.nz > 1 && c->kf[2] != 1.0)))
+        return fail(c, MHD_EINVAL, "mhd_diagnostics: shell spectra are defined on the 2*pi box only");
+    {
+        // Velocity spectrum and the paper's diagnostics (Omega(t), Rayleigh quotient): u = m/rho is not band-limited, and the spectrum is defined over ALL modes
         // (it sums to 1/2 <|u|^2>), so u^ comes from an unpruned forward transform:
         // x pass into W2 viewed as [3][nz][ny][pxf], then y and z in place.
         CK(launch_velocity3(c->Rf, c->Rg, n, c->st));
@@ -511,18 +562,23 @@ int mhd_diagnostics(mhd_ctx* c, mhd_diag* out, double* ekin_spec, double* emag_s
             a.inner = g.ny * fg.px; a.nk_in = a.nk_out = g.nz;
             CK(launch_fft_axis(g.nz, false, a, c->twz, c->st));
         }
-        CK(launch_spectrum(fg, c->W2, (double*)c->G, c->spec_dev, nshell, c->st));
-        if (c->hydro) CK(cudaMemsetAsync(c->spec_dev + kMaxShell, 0, sizeof(double) * nshell, c->st));
-        else CK(launch_spectrum(sg, c->S + F_BX * g.fieldc, (double*)c->G, c->spec_dev + kMaxShell, nshell, c->st));
+        CK(launch_reduce_curl(fg, c->W2, c->kf[0], c->kf[1], c->kf[2], c->red_partial, c->red_result + 20, c->st));
+        if (c->hydro) CK(cudaMemsetAsync(c->red_result + 24, 0, 2 * sizeof(double), c->st));
+        else CK(launch_reduce_curl(sg, c->S + F_BX * g.fieldc, c->kf[0], c->kf[1], c->kf[2], c->red_partial, c->red_result + 24, c->st));
+        if (nshell > 0) {
+            CK(launch_spectrum(fg, c->W2, (double*)c->G, c->spec_dev, nshell, c->st));
+            if (c->hydro) CK(cudaMemsetAsync(c->spec_dev + kMaxShell, 0, sizeof(double) * nshell, c->st));
+            else CK(launch_spectrum(sg, c->S + F_BX * g.fieldc, (double*)c->G, c->spec_dev + kMaxShell, nshell, c->st));
+        }
     }
     if (!c->hydro) {
-        CK(launch_divb_spec(sg, c->S + F_BX * g.fieldc, c->G, c->st));
+        CK(launch_divb_spec(sg, c->S + F_BX * g.fieldc, c->G, c->kf[0], c->kf[1], c->kf[2], c->st));
         CK(inverse_fields(c, c->G, 1, c->Rg));
         CK(launch_reduce_maxabs(c->Rg, n, c->red_partial, c->red_result + 16, c->st));
     } else {
         CK(cudaMemsetAsync(c->red_result + 16, 0, 2 * sizeof(double), c->st));
     }
-    double r[32];
+    double r[32];   // [0..10] field sums + bad flag, [16..17] max|div B| + bad flag, [20..21] curl u / u sums, [24..25] curl B / B sums
     CK(cudaMemcpyAsync(r, c->red_result, sizeof(r), cudaMemcpyDeviceToHost, c->st));
     if (nshell > 0) {
         CK(cudaMemcpyAsync(ekin_spec, c->spec_dev, sizeof(double) * nshell, cudaMemcpyDeviceToHost, c->st));
@@ -534,6 +590,11 @@ int mhd_diagnostics(mhd_ctx* c, mhd_diag* out, double* ekin_spec, double* emag_s
     out->ekin = r[0] * inv; out->emag = r[1] * inv; out->eiso = c->cs * c->cs * r[2] * inv; out->mass = r[3] * inv;
     for (int i = 0; i < 3; ++i) { out->mom[i] = r[4 + i] * inv; out->bmean[i] = r[7 + i] * inv; }
     out->max_divb = r[16];
+    out->enstrophy = r[20] * inv * inv; out->u2 = r[21] * inv * inv; out->current2 = r[24] * inv * inv;
+    {
+        const double den = out->u2 + out->emag;     // <|u|^2> + 1/2 <|B|^2>
+        out->rayleigh_q = den > 0.0 ? (out->enstrophy + 0.5 * out->current2) / den : 0.0;
+    }
     const bool bad = r[RED_NSUM] != 0.0 || r[17] != 0.0;
     if (bad) return fail(c, MHD_ENONFINITE, "non-finite value or rho <= 0 in the state");
     return MHD_OK;

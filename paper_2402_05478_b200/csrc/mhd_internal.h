@@ -63,7 +63,9 @@ struct StageArgs {
     const double2* G;             // 12 (9 hydro) flux fields
     double2* H;                   // AB2: previous RHS (7 fields).  RK4: S0 (state at step start)
     double2* Acc;                 // RK4: accumulator (7 fields)
+    const double2* F;             // masked transform of the body force (3 fields) or nullptr
     double nu, eta, cs2, dt;
+    double kfx, kfy, kfz;         // 2*pi/L per axis: physical wavenumber = factor * integer index
     int mode;
     int hydro;
 };
@@ -74,7 +76,9 @@ cudaError_t launch_momentum(const double* rho, const double* ux, const double* u
                             long long npts, cudaStream_t st);            // m_i = rho*u_i into 3 consecutive fields
 cudaError_t launch_velocity(const double* f, double* ux, double* uy, double* uz, long long npts, cudaStream_t st);
 cudaError_t launch_velocity3(const double* f, double* u3, long long npts, cudaStream_t st);  // u = m/rho, 3 consecutive
-cudaError_t launch_divb_spec(const SpecGeom& g, const double2* B, double2* out, cudaStream_t st);  // i k.B^
+cudaError_t launch_divb_spec(const SpecGeom& g, const double2* B, double2* out, double kfx, double kfy, double kfz, cudaStream_t st);  // i k.B^
+// results[0] = sum_k w |k x V^|^2, results[1] = sum_k w |V^|^2 over the full spectrum (w = 1 on self-conjugate x planes, else 2)
+cudaError_t launch_reduce_curl(const SpecGeom& g, const double2* V3, double kfx, double kfy, double kfz, double* partial, double* results, cudaStream_t st);
 cudaError_t launch_zero(void* p, size_t bytes, cudaStream_t st);
 
 // reductions: results[0..9] = sums of (ekin, emag, rho ln rho, rho, mx, my, mz, bx, by, bz) terms, results[10] = bad flag

@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(kThreads) stage_kernel(StageArgs a) {
         if (jx >= g.nkx) continue;
         const long long row = idx / g.px;
         const int jy = (int)(row % g.nky), jz = (int)(row / g.nky);
-        const double kx = (double)jx, ky = wavenum(jy, g.nky), kz = wavenum(jz, g.nkz);
+        const double kx = a.kfx * (double)jx, ky = a.kfy * wavenum(jy, g.nky), kz = a.kfz * wavenum(jz, g.nkz);
         const double k2 = kx * kx + ky * ky + kz * kz;
 
         double2 S[NFIELD], R[NFIELD];
@@ -136,6 +136,10 @@ __global__ void __launch_bounds__(kThreads) stage_kernel(StageArgs a) {
             R[F_MY] = make_double2(dy - vk * uy.x, -dx - vk * uy.y);
             dx = kx * txz.x + ky * tyz.x + kz * (tzz.x + pr.x); dy = kx * txz.y + ky * tyz.y + kz * (tzz.y + pr.y);
             R[F_MZ] = make_double2(dy - vk * uz.x, -dx - vk * uz.y);
+            if (a.F) {   // eq. (2): + f (steady body force; stored pruned, i.e. already masked)
+                const double2 fx = a.F[idx], fy = a.F[F + idx], fz = a.F[2 * F + idx];
+                R[F_MX].x += fx.x; R[F_MX].y += fx.y; R[F_MY].x += fy.x; R[F_MY].y += fy.y; R[F_MZ].x += fz.x; R[F_MZ].y += fz.y;
+            }
         }
         // eq. (4): R_B = i k x E^ - eta k^2 B^
         if (!HYDRO) {
@@ -179,7 +183,7 @@ cudaError_t launch_stage(const StageArgs& a, cudaStream_t st) {
 }
 
 // ---- S5: diagnostics -----------------------------------------------------------------------------
-__global__ void divb_spec_kernel(SpecGeom g, const double2* __restrict__ B, double2* __restrict__ out) {
+__global__ void divb_spec_kernel(SpecGeom g, const double2* __restrict__ B, double2* __restrict__ out, double kfx, double kfy, double kfz) {
     const long long F = g.field;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < F; idx += (long long)gridDim.x * blockDim.x) {
         const int jx = (int)(idx % g.px);
@@ -187,7 +191,7 @@ __global__ void divb_spec_kernel(SpecGeom g, const double2* __restrict__ B, doub
         const int jy = (int)(row % g.nky), jz = (int)(row / g.nky);
         double2 r = make_double2(0.0, 0.0);
         if (jx < g.nkx) {
-            const double kx = (double)jx, ky = wavenum(jy, g.nky), kz = wavenum(jz, g.nkz);
+            const double kx = kfx * (double)jx, ky = kfy * wavenum(jy, g.nky), kz = kfz * wavenum(jz, g.nkz);
             const double2 bx = B[idx], by = B[F + idx], bz = B[2 * F + idx];
             const double dx = kx * bx.x + ky * by.x + kz * bz.x, dy = kx * bx.y + ky * by.y + kz * bz.y;
             r = make_double2(-dy, dx);   // i * (k.B^)
@@ -195,10 +199,10 @@ __global__ void divb_spec_kernel(SpecGeom g, const double2* __restrict__ B, doub
         out[idx] = r;
     }
 }
-cudaError_t launch_divb_spec(const SpecGeom& g, const double2* B, double2* out, cudaStream_t st) {
+cudaError_t launch_divb_spec(const SpecGeom& g, const double2* B, double2* out, double kfx, double kfy, double kfz, cudaStream_t st) {
     long long blocks = (g.field + kThreads - 1) / kThreads;
     if (blocks > kGridStream) blocks = kGridStream;
-    divb_spec_kernel<<<(unsigned)blocks, kThreads, 0, st>>>(g, B, out);
+    divb_spec_kernel<<<(unsigned)blocks, kThreads, 0, st>>>(g, B, out, kfx, kfy, kfz);
     count_launch();
     return cudaGetLastError();
 }
@@ -314,6 +318,40 @@ cudaError_t launch_reduce_maxabs(const double* a, long long npts, double* partia
     reduce_maxabs_kernel<<<RED_BLOCKS, kThreads, 0, st>>>(a, npts, partial);
     count_launch();
     reduce_final_max_kernel<<<1, kThreads, 0, st>>>(partial, RED_BLOCKS, result);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// ---- paper diagnostics: sum_k w |k x V^|^2 and sum_k w |V^|^2 over a 3-component spectrum (Parseval) ---------
+// Omega(t) = <|curl u|^2> and the terms of the Rayleigh quotient eq. (14).
+// Half-spectrum entries with 0 < kx < nx/2 stand for two modes (w = 2).  Fixed grid + fixed tree: deterministic.
+__global__ void __launch_bounds__(kThreads) reduce_curl_kernel(SpecGeom g, const double2* __restrict__ V, double kfx, double kfy, double kfz,
+                                                               double* __restrict__ partial) {
+    __shared__ double sm[2 * (kThreads / 32)];
+    const long long F = g.field;
+    double v[2] = {0.0, 0.0};
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < F; idx += (long long)gridDim.x * blockDim.x) {
+        const int jx = (int)(idx % g.px);
+        if (jx >= g.nkx) continue;
+        const long long row = idx / g.px;
+        const int jy = (int)(row % g.nky), jz = (int)(row / g.nky);
+        const double kx = kfx * (double)jx, ky = kfy * wavenum(jy, g.nky), kz = kfz * wavenum(jz, g.nkz);
+        const double w = (jx == 0 || 2 * jx == g.nx) ? 1.0 : 2.0;
+        const double2 a = V[idx], b = V[F + idx], c = V[2 * F + idx];
+        const double wxr = ky * c.x - kz * b.x, wxi = ky * c.y - kz * b.y;
+        const double wyr = kz * a.x - kx * c.x, wyi = kz * a.y - kx * c.y;
+        const double wzr = kx * b.x - ky * a.x, wzi = kx * b.y - ky * a.y;
+        v[0] += w * (wxr * wxr + wxi * wxi + wyr * wyr + wyi * wyi + wzr * wzr + wzi * wzi);
+        v[1] += w * (a.x * a.x + a.y * a.y + b.x * b.x + b.y * b.y + c.x * c.x + c.y * c.y);
+    }
+    block_sum<2>(v, sm);
+    if (threadIdx.x == 0) { partial[blockIdx.x] = v[0]; partial[gridDim.x + blockIdx.x] = v[1]; }
+}
+cudaError_t launch_reduce_curl(const SpecGeom& g, const double2* V3, double kfx, double kfy, double kfz, double* partial, double* results,
+                               cudaStream_t st) {
+    reduce_curl_kernel<<<RED_BLOCKS, kThreads, 0, st>>>(g, V3, kfx, kfy, kfz, partial);
+    count_launch();
+    reduce_final_sum_kernel<<<1, kThreads, 0, st>>>(partial, RED_BLOCKS, 2, results);
     count_launch();
     return cudaGetLastError();
 }

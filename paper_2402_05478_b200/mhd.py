@@ -15,10 +15,11 @@ LIB_PATH = os.path.join(_HERE, "libmhd_b200.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = 0, -1, -2, -3, -4, -5
 AB2, RK4 = 0, 1
-FLAG_HYDRO, FLAG_NO_DEALIAS = 1, 2
+FLAG_HYDRO, FLAG_NO_DEALIAS, FLAG_FORCING = 1, 2, 4
 
 EXPORTS = [
-    "mhd_workspace_bytes", "mhd_create", "mhd_destroy", "mhd_set_fields", "mhd_set_fields_host", "mhd_step",
+    "mhd_workspace_bytes", "mhd_create", "mhd_destroy", "mhd_set_fields", "mhd_set_fields_host", "mhd_set_box",
+    "mhd_set_forcing", "mhd_set_forcing_host", "mhd_step",
     "mhd_get_fields", "mhd_get_fields_host", "mhd_diagnostics", "mhd_strerror", "mhd_last_error",
     "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy",
     "mhd_launch_count", "mhd_profile_kernel_count", "mhd_profile_kernel_name", "mhd_profile_begin", "mhd_profile_end",
@@ -28,7 +29,8 @@ EXPORTS = [
 class Diag(C.Structure):
     _fields_ = [("step", C.c_longlong), ("time", C.c_double), ("ekin", C.c_double), ("emag", C.c_double),
                 ("eiso", C.c_double), ("mass", C.c_double), ("mom", C.c_double * 3),
-                ("bmean", C.c_double * 3), ("max_divb", C.c_double)]
+                ("bmean", C.c_double * 3), ("max_divb", C.c_double),
+                ("enstrophy", C.c_double), ("current2", C.c_double), ("u2", C.c_double), ("rayleigh_q", C.c_double)]
 
 
 class MhdError(RuntimeError):
@@ -58,6 +60,9 @@ def lib():
         L.mhd_destroy.restype = None
         for name in ("mhd_set_fields", "mhd_set_fields_host", "mhd_get_fields", "mhd_get_fields_host"):
             getattr(L, name).argtypes = [_vp] * 8
+        L.mhd_set_box.argtypes = [_vp, C.c_double, C.c_double, C.c_double]
+        L.mhd_set_forcing.argtypes = [_vp] * 4
+        L.mhd_set_forcing_host.argtypes = [_vp] * 4
         L.mhd_step.argtypes = [_vp, C.c_int]
         L.mhd_diagnostics.argtypes = [_vp, C.POINTER(Diag), _vp, _vp, C.c_int]
         L.mhd_strerror.restype = C.c_char_p
@@ -227,6 +232,20 @@ class Solver:
         self._check(lib().mhd_get_fields_host(self._h, *ptrs), "mhd_get_fields_host")
         return out
 
+    def set_box(self, lx, ly, lz):
+        self._check(lib().mhd_set_box(self._h, float(lx), float(ly), float(lz)), "mhd_set_box")
+
+    def set_forcing(self, fx=None, fy=None, fz=None):
+        """steady body force f of eq. (2): CUDA tensors, or None x 3 to switch it off (needs FLAG_FORCING)."""
+        ptrs = [_dev_ptr(t, self.npts, n) for t, n in zip((fx, fy, fz), ("fx", "fy", "fz"))]
+        self._before()
+        self._check(lib().mhd_set_forcing(self._h, *ptrs), "mhd_set_forcing")
+        self._after()
+
+    def set_forcing_host(self, fx=None, fy=None, fz=None):
+        ptrs = [_host_ptr(a, self.npts, n) for a, n in zip((fx, fy, fz), ("fx", "fy", "fz"))]
+        self._check(lib().mhd_set_forcing_host(self._h, *ptrs), "mhd_set_forcing_host")
+
     def step(self, n=1):
         self._check(lib().mhd_step(self._h, int(n)), "mhd_step")
 
@@ -237,7 +256,8 @@ class Solver:
         rc = self._check(lib().mhd_diagnostics(self._h, C.byref(d), _vp(ek.ctypes.data), _vp(em.ctypes.data), int(nshell)),
                          "mhd_diagnostics", allow=(ENONFINITE,))
         out = dict(step=d.step, time=d.time, ekin=d.ekin, emag=d.emag, eiso=d.eiso, mass=d.mass,
-                   mom=np.array(d.mom[:]), bmean=np.array(d.bmean[:]), max_divb=d.max_divb, rc=rc)
+                   mom=np.array(d.mom[:]), bmean=np.array(d.bmean[:]), max_divb=d.max_divb, rc=rc,
+                   enstrophy=d.enstrophy, current2=d.current2, u2=d.u2, rayleigh_q=d.rayleigh_q)
         if nshell > 0:
             out["ekin_spec"] = ek[:nshell].copy()
             out["emag_spec"] = em[:nshell].copy()

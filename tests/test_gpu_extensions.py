@@ -1,0 +1,153 @@
+"""GPU parity for SURVEY.md §8(f) rows #2 and #3: box lengths, the steady body force of eq. (2), and the paper's
+diagnostics (Omega(t) PAPER.md:201, Rayleigh quotient eq. (14)), CUDA library vs CPU oracle."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2402_05478_b200 import inputs
+
+TWO_PI = 2 * np.pi
+PER_STEP, ENERGY = 1e-11, 1e-10
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2402_05478_b200 import mhd
+    mhd.lib()
+    return mhd
+
+
+def rel(got, want):
+    g = np.concatenate([np.asarray(a).ravel() for a in got])
+    w = np.concatenate([np.asarray(a).ravel() for a in want])
+    return float(np.linalg.norm(g - w) / np.linalg.norm(w))
+
+
+def both(gpu, ref, shape, f, nu, eta, cs, dt, integrator=0, flags=0, box=None, force=None):
+    import torch
+    nz, ny, nx = shape
+    o = ref.RefSolver(nx, ny, nz, nu, eta, cs, dt, integrator=integrator, flags=flags & 3)
+    g = gpu.Solver(nx, ny, nz, nu, eta, cs, dt, integrator=integrator, flags=flags)
+    if box is not None:
+        o.set_box(*box)
+        g.set_box(*box)
+    if force is not None:
+        o.set_forcing(*force)
+        g.set_forcing(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in force])
+    o.set_fields(*f)
+    g.set_fields(*[torch.from_numpy(a).cuda() for a in f])
+    return o, g
+
+
+def fields_err(g, o):
+    got = [t.cpu().numpy() for t in g.get_fields()]
+    want = o.get_fields()
+    return max(rel(got[0:1], want[0:1]), rel(got[1:4], want[1:4]), rel(got[4:7], want[4:7]))
+
+
+def diag_close(dg, do):
+    for k in ("ekin", "emag", "eiso", "mass", "enstrophy", "current2", "u2", "rayleigh_q"):
+        assert abs(dg[k] - do[k]) <= ENERGY * max(abs(do[k]), 1e-300) + (1e-15 if k == "eiso" else 0.0), (k, dg[k], do[k])
+    assert abs(dg["max_divb"] - do["max_divb"]) <= 1e-11
+
+
+@pytest.mark.parametrize("integrator", [0, 1])
+def test_stretched_box_matches_oracle(gpu, ref, integrator):
+    shape = (16, 24, 32)
+    f = inputs.smooth_random_state(32, 24, 16, seed=31)
+    o, g = both(gpu, ref, shape, f, 2e-3, 3e-3, 1.2, 5e-4, integrator=integrator, box=(1.0, 2.0, 3.0))
+    o.step(1); g.step(1)
+    assert fields_err(g, o) <= PER_STEP
+    o.step(9); g.step(9)                      # AB2: steps 4.. replay the captured graph with the box baked in
+    assert fields_err(g, o) <= 1e-12
+    diag_close(g.diagnostics(), o.diagnostics())
+
+
+def test_set_box_after_graph_capture_takes_effect(gpu, ref):
+    shape = (16, 16, 16)
+    f = inputs.smooth_random_state(16, 16, 16, seed=32)
+    o, g = both(gpu, ref, shape, f, 1e-2, 1e-2, 1.0, 1e-3)
+    o.step(6); g.step(6)
+    o.set_box(TWO_PI, 3.0, TWO_PI); g.set_box(TWO_PI, 3.0, TWO_PI)
+    o.step(6); g.step(6)
+    assert fields_err(g, o) <= 1e-12
+
+
+@pytest.mark.parametrize("integrator", [0, 1])
+def test_forced_run_matches_oracle(gpu, ref, integrator):
+    """forced ABC flow of App. B eq. (B3) (alpha = 0.1) on a smooth random MHD state."""
+    n = 32
+    shape = (n, n, n)
+    f = inputs.smooth_random_state(n, n, n, seed=33)
+    force = [0.1 * c for c in inputs.abc_flow(n, n, n)]
+    o, g = both(gpu, ref, shape, f, 1e-2, 1e-2, 1.0, 1e-3, integrator=integrator, flags=gpu.FLAG_FORCING, force=force)
+    o.step(1); g.step(1)
+    assert fields_err(g, o) <= PER_STEP
+    o.step(11); g.step(11)
+    assert fields_err(g, o) <= 1e-12
+    diag_close(g.diagnostics(16), o.diagnostics(16))
+    # switching the force off (after graph capture) is honoured too
+    o.set_forcing(None, None, None); g.set_forcing(None, None, None)
+    o.step(5); g.step(5)
+    assert fields_err(g, o) <= 1e-12
+
+
+def test_forced_2d_hydro_orszag_tang_b2(gpu, ref):
+    """App. B eq. (B2): 2-D flow forced with its own shape, hydro flag, host-buffer forcing call."""
+    n = 64
+    x = TWO_PI * np.arange(n) / n
+    Y, X = np.meshgrid(x, x, indexing="ij")
+    ux = (-np.sin(Y))[None].copy(); uy = np.sin(X)[None].copy()
+    one = np.ones((1, n, n)); zero = np.zeros((1, n, n))
+    import torch
+    fl = gpu.FLAG_FORCING | gpu.FLAG_HYDRO
+    o = ref.RefSolver(n, n, 1, 5e-3, 0.0, 2.0, 1e-3, flags=1)
+    g = gpu.Solver(n, n, 1, 5e-3, 0.0, 2.0, 1e-3, flags=fl)
+    o.set_forcing(0.1 * ux, 0.1 * uy, zero)
+    g.set_forcing_host(np.ascontiguousarray(0.1 * ux), np.ascontiguousarray(0.1 * uy), zero)
+    o.set_fields(one, ux, uy, zero)
+    g.set_fields(*[torch.from_numpy(a).cuda() for a in (one, ux, uy, zero)])
+    o.step(40); g.step(40)
+    got = [t.cpu().numpy() for t in g.get_fields()]
+    want = o.get_fields()
+    assert rel(got[0:4], want[0:4]) <= 1e-12
+    diag_close(g.diagnostics(), o.diagnostics())
+
+
+def test_forcing_needs_the_flag_and_spectra_need_the_2pi_box(gpu):
+    import torch
+    s = gpu.Solver(16, 16, 16, 0.01, 0.01, 1.0, 1e-3)
+    z = torch.zeros((16, 16, 16), dtype=torch.float64, device="cuda")
+    with pytest.raises(gpu.MhdError) as e:
+        s.set_forcing(z, z, z)
+    assert e.value.code == gpu.ESTATE
+    with pytest.raises(gpu.MhdError):
+        s.set_box(-1.0, 1.0, 1.0)
+    s.set_box(1.0, TWO_PI, TWO_PI)
+    s.set_fields(z + 1.0, z, z, z, z, z, z)
+    with pytest.raises(gpu.MhdError) as e:
+        s.diagnostics(8)
+    assert e.value.code == gpu.EINVAL
+    assert s.diagnostics(0)["rc"] == 0
+
+
+def test_paper_diagnostics_on_config1_and_closed_forms(gpu, ref):
+    import torch
+    cfg = inputs.config1()
+    o = ref.RefSolver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
+    g = gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
+    o.set_fields(*cfg.arrays()); g.set_fields(*[torch.from_numpy(a).cuda() for a in cfg.arrays()])
+    o.step(5); g.step(5)
+    diag_close(g.diagnostics(), o.diagnostics())
+    # Beltrami closed form on the GPU alone: ABC flow and field, Q = k0^2 (eq. 14 with curl u = k0 u)
+    n = 32
+    u = inputs.abc_flow(n, n, n, k0=2.0, u0=0.7)
+    b = inputs.abc_flow(n, n, n, k0=2.0, u0=0.2)
+    s = gpu.Solver(n, n, n, 0.01, 0.01, 1.0, 1e-3)
+    s.set_fields(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in [np.ones((n, n, n))] + u + b])
+    d = s.diagnostics()
+    assert abs(d["enstrophy"] - 4 * 3 * 0.49) <= 1e-12 and abs(d["rayleigh_q"] - 4.0) <= 1e-12
