@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmhd_b200.so")
-SOURCES = ["fft_kernels.cu", "xfused_kernel.cu", "mhd_kernels.cu", "mhd_api.cu"]
+SOURCES = ["fft_kernels.cu", "xfused_kernel.cu", "zstage_kernel.cu", "mhd_kernels.cu", "mhd_api.cu"]
 HEADERS = ["fft_core.cuh", "mhd_internal.h"]
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
