@@ -303,6 +303,62 @@ def run_gpu(args):
     return 0
 
 
+def run_fft_sweep(args):
+    """--workload fft: BASELINE config 5, batched 3-D R2C + C2R of 7 fields; effective GB/s = 2 F batch / t
+    (input read once + output written once) against the measured copy peak, round-trip error, and cuFFT
+    (torch.fft, never on the product path) as the one permitted reference line."""
+    import torch
+    from paper_2402_05478_b200 import mhd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, peak_src = measured_peak()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    sweep, l0 = [], mhd.launch_count()
+    for n in [int(v) for v in args.fft_sizes.split(",")]:
+        batch = 7
+        gen = torch.Generator(device=dev); gen.manual_seed(1005)
+        a = torch.rand((batch, n, n, n), dtype=torch.float64, device=dev, generator=gen) * 2.0 - 1.0
+        plan = mhd.FftPlan(n, n, n, batch, stream=torch.cuda.current_stream(dev))
+        spec = plan.r2c(a)
+        back = plan.c2r(spec)
+        err = float(torch.linalg.norm(back - a) / torch.linalg.norm(a))
+
+        def timed(fn, reps=5):
+            ts = []
+            for it in range(3 + reps):
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+                if it >= 3:
+                    ts.append(e0.elapsed_time(e1))
+            return statistics.median(ts)
+        t_r2c = timed(lambda: plan.r2c(a, out=spec))
+        t_c2r = timed(lambda: plan.c2r(spec, out=back))
+        fr, fc = 8.0 * n ** 3 * batch, 16.0 * (n // 2 + 1) * n * n * batch
+        row = {"n": n, "batch": batch, "r2c_ms": t_r2c, "c2r_ms": t_c2r, "roundtrip_rel_err": err,
+               "r2c_eff_gbs": (fr + fc) / 1e9 / (t_r2c * 1e-3), "c2r_eff_gbs": (fr + fc) / 1e9 / (t_c2r * 1e-3)}
+        row["r2c_frac"] = row["r2c_eff_gbs"] / peak
+        row["c2r_frac"] = row["c2r_eff_gbs"] / peak
+        del plan, back
+        try:   # reference line only: cuFFT through torch.fft
+            t_ref = timed(lambda: torch.fft.rfftn(a, dim=(1, 2, 3)), reps=3)
+            row["cufft_r2c_ms"] = t_ref
+        except Exception as ex:   # out of memory at the largest size is not an error of this library
+            row["cufft_r2c_ms"] = None
+            row["cufft_note"] = type(ex).__name__
+        del a, spec
+        torch.cuda.empty_cache()
+        sweep.append(row)
+    line = {"metric": "fft_effective_gbs", "unit": "GB/s", "n_gpus": 1, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config5: batched 3-D R2C + C2R, batch 7, uniform[-1,1) reals", "l2": "256 MB flush between iterations"},
+            "peak": peak, "peak_source": peak_src, "sweep": sweep, "gpu_launches": mhd.launch_count() - l0,
+            "value": max(r["r2c_eff_gbs"] for r in sweep)}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def load_traffic():
     """per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per kernel class from the committed
     ncu summary profiles/traffic.csv (kernel,bytes_per_launch); empty if absent."""
@@ -329,10 +385,14 @@ def main(argv=None):
     ap.add_argument("--ref-n", type=int, default=128, help="grid size of the bounded sample the reference arm times")
     ap.add_argument("--cpu-n", type=int, default=192, help="grid size of the bounded cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="step", choices=["step", "fft"], help="step: the 512^3 MHD step (default); fft: the config-5 FFT sweep")
+    ap.add_argument("--fft-sizes", default="128,256,512,768")
     args = ap.parse_args(argv)
     if args.steps < 1:
         raise SystemExit("--steps must be >= 1")
-    return run_reference(args) if args.impl == "reference" else run_gpu(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_fft_sweep(args) if args.workload == "fft" else run_gpu(args)
 
 
 if __name__ == "__main__":

@@ -13,6 +13,8 @@
 #include "mhd_internal.h"
 #include "fft_core.cuh"
 
+#include <stdlib.h>
+
 namespace mhd {
 using namespace mhdfft;
 
@@ -201,6 +203,8 @@ cudaError_t launch_fft_axis(int n, bool inverse, const AxisArgs& a, const double
 }
 
 cudaError_t launch_fft_rows(int n, bool inverse, const RowArgs& a, const double2* tw, cudaStream_t st) {
+    static const bool legacy = getenv("MHD_LEGACY_XROWS") != nullptr;
+    if (!legacy && xfused_supported(n)) return launch_xrows(n, inverse, a, tw, st);   // coalesced team kernel (xfused_kernel.cu)
     switch (n) {
 #define X(N_) case N_: return launch_rows_n<N_>(inverse, a, tw, st);
         MHD_FOR_EACH_N(X)

@@ -339,7 +339,9 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     c->integrator = integrator; c->flags = flags; c->hydro = (flags & MHD_FLAG_HYDRO) ? 1 : 0;
     c->st = (cudaStream_t)stream; c->ws = (char*)workspace; c->L = L;
     c->xfuse = xfused_supported(nx) && getenv("MHD_NO_XFUSE") == nullptr;
-    c->zfuse = nz > 1 && zstage_supported(nz) && getenv("MHD_NO_ZFUSE") == nullptr;
+    // z forward pass fused with the stage: correct (parity-tested) but, at one 512-thread CTA per SM, 8 % slower than the two
+    // separate kernels at 512^3 (4.56 vs 4.22 ms, profiles/r01c_zstage.md); opt-in until it wins
+    c->zfuse = nz > 1 && zstage_supported(nz) && getenv("MHD_ZFUSE") != nullptr;
     c->prof_ev = new (std::nothrow) std::vector<cudaEvent_t>[K_NCLASS];
     if (!c->prof_ev) { delete c; return MHD_ENOMEM; }
     c->twx = (double2*)(c->ws + L.twx); c->twy = (double2*)(c->ws + L.twy); c->twz = (double2*)(c->ws + L.twz);

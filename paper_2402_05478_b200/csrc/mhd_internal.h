@@ -39,6 +39,8 @@ struct XFusedArgs {
     double scale;             // 1/(nx*ny*nz), applied to the inverse transforms
 };
 bool xfused_supported(int n);
+// stand-alone x pass (row pairs) on the fused kernel's team machinery; n must satisfy xfused_supported(n)
+cudaError_t launch_xrows(int n, bool inverse, const RowArgs& a, const double2* tw, cudaStream_t st);
 cudaError_t launch_xfused(int n, const XFusedArgs& a, int hydro, const double2* tw, cudaStream_t st);
 
 // ---- pointwise / spectral kernels (mhd_kernels.cu) ------------------------------------------

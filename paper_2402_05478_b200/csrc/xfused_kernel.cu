@@ -413,6 +413,151 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Stand-alone x pass on the same team machinery: pairs of real rows <-> pairs of half-spectrum rows (mhd_fft_r2c /
+// mhd_fft_c2r of BASELINE config 5, mhd_set_fields, mhd_get_fields, diagnostics).  One team per row pair; consecutive
+// lanes touch consecutive x (or kx), so every global access is a full line.  Little per-thread state => 256-thread CTAs,
+// several per SM; persistent so the twiddle tables are built once per CTA.
+template <int N> struct XRowCfg {
+    static constexpr int TP = Plan<N>::TP;
+    static constexpr int THREADS = (TP >= 128) ? 256 : 128 < TP ? TP : (N >= 256 ? 256 : 128);
+    static constexpr int TEAMS = THREADS / TP;
+    static constexpr size_t SMEM = sizeof(cplx) * ((size_t)2 * XCfg<N>::BUF * TEAMS + (XCfg<N>::NTW > 0 ? XCfg<N>::NTW : 1));
+};
+
+template <int N, bool INV>
+__global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, const cplx* __restrict__ tw) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    using PL = Plan<N>;
+    using CF = XCfg<N>;
+    using RC = XRowCfg<N>;
+    constexpr int TP = PL::TP, E = 8;
+    constexpr int RL = PL::radix(PL::NP - 1);
+    const int team = threadIdx.x / TP, i = threadIdx.x % TP;
+    cplx* const smbase = reinterpret_cast<cplx*>(smraw);
+    cplx* const stw = smbase + (size_t)2 * CF::BUF * RC::TEAMS;
+    cplx* bufA = smbase + (size_t)team * 2 * CF::BUF;
+    cplx* bufB = bufA + CF::BUF;
+    const int nkx = a.nkx;
+    {
+        int P = PL::radix(0);
+#pragma unroll
+        for (int s = 1; s < PL::NP; ++s) {
+            const int R = PL::radix(s), off = CF::tw_offset(s);
+            for (int e = threadIdx.x; e < (R - 1) * P; e += blockDim.x) {
+                const int q = e / P + 1, k = e % P;
+                stw[off + e] = tw[k * q * (N / (P * R))];
+            }
+            P *= R;
+        }
+    }
+    __syncthreads();
+    const long long npairs = (a.nrows + 1) / 2;
+    const long long stride = (long long)gridDim.x * RC::TEAMS;
+    for (long long pr = (long long)blockIdx.x * RC::TEAMS + team; pr - team < npairs; pr += stride) {
+        const bool ok = pr < npairs;
+        const long long r0 = ok ? 2 * pr : 0;
+        cplx* __restrict__ A = a.spec + r0 * a.spec_pitch;
+        cplx* __restrict__ B = A + a.spec_pitch;
+        double* __restrict__ ra = a.real + r0 * a.real_pitch;
+        double* __restrict__ rb = ra + a.real_pitch;
+        cplx v[E];
+        if constexpr (INV) {
+#pragma unroll
+            for (int q = 0; q < E; ++q) {                 // first-pass input k = i + TP*q
+                const int k = i + TP * q;
+                const bool lo = k < nkx, hi = (N - k) < nkx;
+                const int idx = lo ? k : N - k;
+                cplx x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
+                if (ok && (lo || hi)) { x = A[idx]; y = B[idx]; }
+                if (k == 0 || 2 * k == N) { x.y = 0.0; y.y = 0.0; }                 // self-conjugate modes: Im ignored
+                v[q] = lo ? make_double2(x.x - y.y, x.y + y.x) : make_double2(x.x + y.y, y.x - x.y);
+            }
+            XPass<N, true, 0, 1>::run(v, bufA, bufB, i, team, stw);
+            if (odd_exchanges<N>()) { cplx* t = bufA; bufA = bufB; bufB = t; }
+            const double s = a.scale;
+            if (ok) {
+#pragma unroll
+                for (int m = 0; m < E / RL; ++m)
+#pragma unroll
+                    for (int q = 0; q < RL; ++q) {
+                        const int x = i + TP * (m + q * (E / RL));
+                        ra[x] = v[m * RL + q].x * s;
+                        rb[x] = v[m * RL + q].y * s;
+                    }
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < E; ++q) v[q] = ok ? make_double2(ra[i + TP * q], rb[i + TP * q]) : make_double2(0.0, 0.0);
+            XPass<N, false, 0, 1>::run(v, bufA, bufB, i, team, stw);
+            if (odd_exchanges<N>()) { cplx* t = bufA; bufA = bufB; bufB = t; }
+#pragma unroll
+            for (int m = 0; m < E / RL; ++m)
+#pragma unroll
+                for (int q = 0; q < RL; ++q) {
+                    const int t = m + q * (E / RL);
+                    if (t >= 1 && (TP * (t + 1) > N - nkx)) bufA[N - (i + TP * t)] = v[m * RL + q];
+                }
+            team_sync<TP>(team);
+            const double s = 0.5 * a.scale;
+            if (ok) {
+#pragma unroll
+                for (int m = 0; m < E / RL; ++m)
+#pragma unroll
+                    for (int q = 0; q < RL; ++q) {
+                        const int t = m + q * (E / RL);
+                        const int k = i + TP * t;
+                        if (t <= E / 2 && k < nkx) {
+                            const cplx zk = v[m * RL + q];
+                            const cplx zm = (k == 0) ? zk : bufA[k];
+                            A[k] = make_double2(s * (zk.x + zm.x), s * (zk.y - zm.y));
+                            B[k] = make_double2(s * (zk.y + zm.y), s * (zm.x - zk.x));
+                        }
+                    }
+            }
+            { cplx* t = bufA; bufA = bufB; bufB = t; }
+        }
+    }
+}
+
+template <int N> static cudaError_t launch_xrows_n(bool inverse, const RowArgs& a, const cplx* tw, cudaStream_t st) {
+    if constexpr (Plan<N>::E != 8) {
+        return cudaErrorInvalidValue;
+    } else {
+        using RC = XRowCfg<N>;
+        static int sms = 0;
+        if (sms == 0) {
+            int dev = 0;
+            cudaError_t e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(xrows_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(xrows_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
+            if (e != cudaSuccess) { sms = 0; return e; }
+        }
+        const long long groups = ((a.nrows + 1) / 2 + RC::TEAMS - 1) / RC::TEAMS;
+        const long long cap = (long long)sms * 8;             // persistent; more CTAs than can be resident simply queue
+        const unsigned blocks = (unsigned)(groups < cap ? groups : cap);
+        if (inverse) xrows_kernel<N, true><<<blocks, RC::THREADS, RC::SMEM, st>>>(a, tw);
+        else xrows_kernel<N, false><<<blocks, RC::THREADS, RC::SMEM, st>>>(a, tw);
+        count_launch();
+        return cudaGetLastError();
+    }
+}
+
+cudaError_t launch_xrows(int n, bool inverse, const RowArgs& a, const double2* tw, cudaStream_t st) {
+    switch (n) {
+        case 8: return launch_xrows_n<8>(inverse, a, tw, st);
+        case 16: return launch_xrows_n<16>(inverse, a, tw, st);
+        case 32: return launch_xrows_n<32>(inverse, a, tw, st);
+        case 64: return launch_xrows_n<64>(inverse, a, tw, st);
+        case 128: return launch_xrows_n<128>(inverse, a, tw, st);
+        case 256: return launch_xrows_n<256>(inverse, a, tw, st);
+        case 512: return launch_xrows_n<512>(inverse, a, tw, st);
+        case 1024: return launch_xrows_n<1024>(inverse, a, tw, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
 template <int N> static cudaError_t launch_xfused_n(const XFusedArgs& a, int hydro, const cplx* tw, cudaStream_t st) {
     if constexpr (Plan<N>::E != 8) {
         return cudaErrorInvalidValue;

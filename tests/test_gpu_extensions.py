@@ -151,3 +151,28 @@ def test_paper_diagnostics_on_config1_and_closed_forms(gpu, ref):
     s.set_fields(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in [np.ones((n, n, n))] + u + b])
     d = s.diagnostics()
     assert abs(d["enstrophy"] - 4 * 3 * 0.49) <= 1e-12 and abs(d["rayleigh_q"] - 4.0) <= 1e-12
+
+
+@pytest.mark.parametrize("integrator,hydro", [(0, False), (1, False), (0, True)])
+def test_fused_z_forward_stage_kernel_matches_oracle(gpu, ref, integrator, hydro, monkeypatch):
+    """the opt-in fused z-forward + stage kernel (zstage_kernel.cu, MHD_ZFUSE=1): same results as the oracle,
+    with forcing and a stretched box, Euler start + steady AB2 (graph replay) or RK4."""
+    import torch
+    monkeypatch.setenv("MHD_ZFUSE", "1")
+    shape = (32, 16, 64)
+    f = inputs.smooth_random_state(64, 16, 32, seed=41, hydro=hydro)
+    force = [0.05 * np.cos(np.arange(64) * TWO_PI / 64)[None, None, :] * np.ones(shape), np.zeros(shape), 0.02 * np.ones(shape)]
+    flags = gpu.FLAG_FORCING | (gpu.FLAG_HYDRO if hydro else 0)
+    o, g = both(gpu, ref, shape, f, 3e-3, 2e-3, 1.1, 1e-3, integrator=integrator, flags=flags, box=(TWO_PI, 3.0, 5.0), force=force)
+    launches0 = gpu.launch_count()
+    o.step(1); g.step(1)
+    got = [t.cpu().numpy() for t in g.get_fields()]
+    want = o.get_fields()
+    assert max(rel(got[0:1], want[0:1]), rel(got[1:4], want[1:4])) <= PER_STEP
+    o.step(8); g.step(8)
+    got = [t.cpu().numpy() for t in g.get_fields()]
+    want = o.get_fields()
+    assert max(rel(got[0:1], want[0:1]), rel(got[1:4], want[1:4])) <= 1e-12
+    if not hydro:
+        assert rel(got[4:7], want[4:7]) <= 1e-12
+    assert gpu.launch_count() > launches0
