@@ -128,6 +128,14 @@ struct Cols8 {
     int p;
     __device__ __forceinline__ int operator()(int e) const { return e * 8 + p; }
 };
+// Cols4 : [N][4] complex, 64 bytes per element row.  A quarter-warp (4 pencils x 2 adjacent slots) touches two rows; they
+//         must fall on opposite halves of the 128-byte bank period, so the row index has its lowest bit flipped by the
+//         parity of bits 3 and 6 (adjacent slots differ in bit 0 on reads / radix-8 second-pass writes, in bit 3 on
+//         first-pass writes).
+struct Cols4 {
+    int p;
+    __device__ __forceinline__ int operator()(int e) const { return ((e ^ (((e >> 3) ^ (e >> 6)) & 1)) << 2) + p; }
+};
 struct Padded {
     __device__ __forceinline__ int operator()(int e) const { return e + (e >> 3); }
     __host__ __device__ static constexpr int size(int n) { return n + (n >> 3) + 1; }
@@ -181,6 +189,12 @@ template <int N, bool INV>
 __device__ __forceinline__ void pencil_fft(cplx (&v)[Plan<N>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
     Cols8 lay{p};
     Pass<N, INV, 0, 1, Cols8>::run(v, sm, i, lay, tw);
+}
+// same for 4 pencils side by side (lane = (p = tid & 3, slot))
+template <int N, bool INV>
+__device__ __forceinline__ void pencil_fft4(cplx (&v)[Plan<N>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
+    Cols4 lay{p};
+    Pass<N, INV, 0, 1, Cols4>::run(v, sm, i, lay, tw);
 }
 // same, one pencil per (padded) buffer
 template <int N, bool INV>

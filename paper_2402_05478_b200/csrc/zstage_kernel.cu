@@ -41,11 +41,18 @@ __device__ __forceinline__ int zs_compact(int f, int n, int nk) {
 }
 __device__ __forceinline__ int zs_wavenum_compact(int j, int nk) { return (j < (nk + 1) / 2) ? j : j - nk; }
 
+// columns per tile: 8 (one 128-byte line per row, one 512-thread CTA per SM at N = 512) or 4 (64-byte segments, two
+// 256-thread CTAs per SM).  Measured at 512^3 on B200: 8 -> 4.6 ms, 4 -> 6.1 ms (the 64-byte segments cost more than the
+// second CTA gains), so 8 is the default.
+#ifndef MHD_ZS_CW
+#define MHD_ZS_CW 8
+#endif
 template <int N> struct ZTile {
+    static constexpr int CW = MHD_ZS_CW;
     static constexpr int TP = Plan<N>::TP;
-    static constexpr int G = Tile<N>::G;
-    static constexpr int THREADS = Tile<N>::THREADS;
-    static constexpr int COLS = Tile<N>::COLS;
+    static constexpr int G = (CW * TP >= 128) ? 1 : 128 / (CW * TP);
+    static constexpr int THREADS = CW * TP * G;
+    static constexpr int COLS = CW * G;
     static constexpr size_t SMEM = 3 * (size_t)N * COLS * sizeof(cplx);   // exchange + 2 staging tiles
 };
 
@@ -91,20 +98,20 @@ __device__ __forceinline__ void zs_update_ab2(cplx* __restrict__ Sp, cplx* __res
 
 // AB2STEADY: the stage is known at compile time to be STAGE_AB2
 template <int N, bool HYDRO, bool AB2STEADY>
-__global__ void __launch_bounds__(ZTile<N>::THREADS, 1) zstage_kernel(ZStageArgs a, const cplx* __restrict__ tw) {
+__global__ void __launch_bounds__(ZTile<N>::THREADS, (ZTile<N>::CW == 4 && ZTile<N>::THREADS <= 256) ? 2 : 1) zstage_kernel(ZStageArgs a, const cplx* __restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smraw[];
     using PL = Plan<N>;
     static_assert(PL::E == 8 && PL::radix(0) == 8, "zstage needs 8 points per thread and a radix-8 first pass");
     constexpr int TP = PL::TP, E = 8, RL = PL::radix(PL::NP - 1);
-    constexpr int G = ZTile<N>::G;
-    const int tid = threadIdx.x, p = tid & 7, i = (tid >> 3) % TP, g = tid / (8 * TP);
-    cplx* const ex = reinterpret_cast<cplx*>(smraw) + (size_t)g * N * 8;
-    cplx* const st0 = reinterpret_cast<cplx*>(smraw) + (size_t)(G + g) * N * 8;
-    cplx* const st1 = st0 + (size_t)G * N * 8;
+    constexpr int G = ZTile<N>::G, CW = ZTile<N>::CW;
+    const int tid = threadIdx.x, p = tid & (CW - 1), i = (tid / CW) % TP, g = tid / (CW * TP);
+    cplx* const ex = reinterpret_cast<cplx*>(smraw) + (size_t)g * N * CW;
+    cplx* const st0 = reinterpret_cast<cplx*>(smraw) + (size_t)(G + g) * N * CW;
+    cplx* const st1 = st0 + (size_t)G * N * CW;
     const StageArgs& s = a.st;
     const SpecGeom& geo = s.g;
     const long long F = geo.field;
-    const long long col = (long long)blockIdx.x * ZTile<N>::COLS + g * 8 + p;
+    const long long col = (long long)blockIdx.x * ZTile<N>::COLS + g * CW + p;
     const int jx = (int)(col % geo.px);
     const int jy = (int)(col / geo.px);
     const bool colok = col < a.inner && jx < geo.nkx;
@@ -116,7 +123,7 @@ __global__ void __launch_bounds__(ZTile<N>::THREADS, 1) zstage_kernel(ZStageArgs
         if (colok && field >= 0) {
             const cplx* src = a.W1 + (long long)field * a.w1field + col;
 #pragma unroll
-            for (int q = 0; q < E; ++q) cp_async16(&buf[(i + TP * q) * 8 + p], src + (long long)(i + TP * q) * a.inner);
+            for (int q = 0; q < E; ++q) cp_async16(&buf[(i + TP * q) * CW + p], src + (long long)(i + TP * q) * a.inner);
         }
         cp_async_commit();
     };
@@ -130,7 +137,7 @@ __global__ void __launch_bounds__(ZTile<N>::THREADS, 1) zstage_kernel(ZStageArgs
     };
     // pull the state / history lines this thread will touch in a finish phase into L2 ahead of time (no registers)
     auto prefetch_state = [&](int field) {
-        if (!colok || p != 0) return;            // one lane per 128-byte line
+        if (!colok || p != 0) return;            // one lane per tile row (a 128- or 64-byte segment)
 #pragma unroll
         for (int m = 0; m < E / RL; ++m)
 #pragma unroll
@@ -165,14 +172,14 @@ __global__ void __launch_bounds__(ZTile<N>::THREADS, 1) zstage_kernel(ZStageArgs
             const double ca = (j == 12) ? -ky : kx, cb = (j == 12) ? kx : ky;      // job 12: st0 = Ex, st1 = Ey
 #pragma unroll
             for (int q = 0; q < E; ++q) {
-                const cplx x = colok ? st0[(i + TP * q) * 8 + p] : make_double2(0.0, 0.0);
-                const cplx y = colok ? st1[(i + TP * q) * 8 + p] : make_double2(0.0, 0.0);
+                const cplx x = colok ? st0[(i + TP * q) * CW + p] : make_double2(0.0, 0.0);
+                const cplx y = colok ? st1[(i + TP * q) * CW + p] : make_double2(0.0, 0.0);
                 v[q] = make_double2(ca * x.x + cb * y.x, ca * x.y + cb * y.y);
             }
         } else {
             const cplx* buf = (j < 9 ? ph == 1 : (j != 10)) ? st0 : st1;
 #pragma unroll
-            for (int q = 0; q < E; ++q) v[q] = colok ? buf[(i + TP * q) * 8 + p] : make_double2(0.0, 0.0);
+            for (int q = 0; q < E; ++q) v[q] = colok ? buf[(i + TP * q) * CW + p] : make_double2(0.0, 0.0);
         }
         // ---- refill the slots just read with the tiles of the next jobs ----
         {
@@ -191,7 +198,8 @@ __global__ void __launch_bounds__(ZTile<N>::THREADS, 1) zstage_kernel(ZStageArgs
             if (j == 9) { prefetch_state(F_BX); prefetch_state(F_BY); }
             if (j == 11) prefetch_state(F_BZ);
         }
-        pencil_fft<N, false>(v, ex, i, p, tw);
+        if constexpr (CW == 8) pencil_fft<N, false>(v, ex, i, p, tw);
+        else pencil_fft4<N, false>(v, ex, i, p, tw);
         // ---- consume ----
 #pragma unroll
         for (int m = 0; m < E / RL; ++m)
