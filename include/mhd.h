@@ -119,6 +119,17 @@ int mhd_get_fields_host(mhd_ctx* ctx, double* rho_host, double* ux_host, double*
  * sticky CUDA error. */
 int mhd_diagnostics(mhd_ctx* ctx, mhd_diag* out_host, double* ekin_spec_host, double* emag_spec_host, int nshell);
 
+/* Exact resume (the paper restarts from ASCII dumps; restarting AB2 from grid fields alone would
+ * re-bootstrap with an Euler step).  mhd_get_state copies the spectral state, the integrator history and a small header
+ * (grid, flags, integrator, step count) into state_dev, a caller-owned DEVICE buffer of mhd_state_bytes(ctx) bytes;
+ * mhd_set_state restores them into a context created with the same nx, ny, nz, integrator and flags (MHD_EINVAL
+ * otherwise; it synchronises to read the header).  A run continued after mhd_set_state is bit-identical to the
+ * uninterrupted run.  The blob's layout is internal to this library version.  Box, forcing, nu, eta, cs, dt are NOT
+ * part of the state: set them on the new context as before. */
+size_t mhd_state_bytes(const mhd_ctx* ctx);
+int mhd_get_state(mhd_ctx* ctx, void* state_dev, size_t bytes);
+int mhd_set_state(mhd_ctx* ctx, const void* state_dev, size_t bytes);
+
 const char* mhd_strerror(int code);
 const char* mhd_last_error(const mhd_ctx* ctx);   /* detail of the last failure on this context ("" if none) */
 

@@ -539,6 +539,59 @@ int mhd_get_fields_host(mhd_ctx* c, double* rho, double* ux, double* uy, double*
     return MHD_OK;
 }
 
+namespace {
+struct StateHeader {          // first 256 bytes of the blob
+    unsigned long long magic;
+    int nx, ny, nz, integrator;
+    unsigned flags;
+    int have_fields, have_history;
+    long long step;
+};
+constexpr unsigned long long kStateMagic = 0x4d48443153544154ull;   // "MHD1STAT"
+constexpr size_t kStateHeaderBytes = 256;
+}  // namespace
+
+size_t mhd_state_bytes(const mhd_ctx* c) {
+    if (!c) return 0;
+    return kStateHeaderBytes + 2 * sizeof(double2) * (size_t)c->g.fieldc * NFIELD;      // header + S + H
+}
+
+int mhd_get_state(mhd_ctx* c, void* state, size_t bytes) {
+    if (!c) return MHD_EINVAL;
+    if (!state || bytes < mhd_state_bytes(c)) return fail(c, MHD_EINVAL, "mhd_get_state: buffer missing or too small");
+    if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_get_state before mhd_set_fields");
+    StateHeader h;
+    memset(&h, 0, sizeof(h));
+    h.magic = kStateMagic; h.nx = c->g.nx; h.ny = c->g.ny; h.nz = c->g.nz; h.integrator = c->integrator;
+    h.flags = c->flags & (MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS);
+    h.have_fields = c->have_fields; h.have_history = c->have_history; h.step = c->step;
+    const size_t fb = sizeof(double2) * (size_t)c->g.fieldc * NFIELD;
+    char* d = (char*)state;
+    CK(cudaMemsetAsync(d, 0, kStateHeaderBytes, c->st));
+    CK(cudaMemcpyAsync(d, &h, sizeof(h), cudaMemcpyHostToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));                      // h lives on this stack frame
+    CK(cudaMemcpyAsync(d + kStateHeaderBytes, c->S, fb, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaMemcpyAsync(d + kStateHeaderBytes + fb, c->H, fb, cudaMemcpyDeviceToDevice, c->st));
+    return MHD_OK;
+}
+
+int mhd_set_state(mhd_ctx* c, const void* state, size_t bytes) {
+    if (!c) return MHD_EINVAL;
+    if (!state || bytes < mhd_state_bytes(c)) return fail(c, MHD_EINVAL, "mhd_set_state: buffer missing or too small");
+    StateHeader h;
+    CK(cudaMemcpyAsync(&h, state, sizeof(h), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    if (h.magic != kStateMagic || h.nx != c->g.nx || h.ny != c->g.ny || h.nz != c->g.nz || h.integrator != c->integrator ||
+        h.flags != (c->flags & (MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS)) || !h.have_fields)
+        return fail(c, MHD_EINVAL, "mhd_set_state: the blob was written by a different configuration");
+    const size_t fb = sizeof(double2) * (size_t)c->g.fieldc * NFIELD;
+    const char* d = (const char*)state;
+    CK(cudaMemcpyAsync(c->S, d + kStateHeaderBytes, fb, cudaMemcpyDeviceToDevice, c->st));
+    CK(cudaMemcpyAsync(c->H, d + kStateHeaderBytes + fb, fb, cudaMemcpyDeviceToDevice, c->st));
+    c->have_fields = 1; c->have_history = h.have_history; c->step = h.step;
+    return MHD_OK;
+}
+
 int mhd_diagnostics(mhd_ctx* c, mhd_diag* out, double* ekin_spec, double* emag_spec, int nshell) {
     if (!c) return MHD_EINVAL;
     if (!out || nshell < 0 || nshell > kMaxShell || (nshell > 0 && (!ekin_spec || !emag_spec)))

@@ -20,6 +20,7 @@ FLAG_HYDRO, FLAG_NO_DEALIAS, FLAG_FORCING = 1, 2, 4
 EXPORTS = [
     "mhd_workspace_bytes", "mhd_create", "mhd_destroy", "mhd_set_fields", "mhd_set_fields_host", "mhd_set_box",
     "mhd_set_forcing", "mhd_set_forcing_host", "mhd_step",
+    "mhd_state_bytes", "mhd_get_state", "mhd_set_state",
     "mhd_get_fields", "mhd_get_fields_host", "mhd_diagnostics", "mhd_strerror", "mhd_last_error",
     "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy",
     "mhd_launch_count", "mhd_profile_kernel_count", "mhd_profile_kernel_name", "mhd_profile_begin", "mhd_profile_end",
@@ -64,6 +65,10 @@ def lib():
         L.mhd_set_forcing.argtypes = [_vp] * 4
         L.mhd_set_forcing_host.argtypes = [_vp] * 4
         L.mhd_step.argtypes = [_vp, C.c_int]
+        L.mhd_state_bytes.restype = C.c_size_t
+        L.mhd_state_bytes.argtypes = [_vp]
+        L.mhd_get_state.argtypes = [_vp, _vp, C.c_size_t]
+        L.mhd_set_state.argtypes = [_vp, _vp, C.c_size_t]
         L.mhd_diagnostics.argtypes = [_vp, C.POINTER(Diag), _vp, _vp, C.c_int]
         L.mhd_strerror.restype = C.c_char_p
         L.mhd_strerror.argtypes = [C.c_int]
@@ -245,6 +250,24 @@ class Solver:
     def set_forcing_host(self, fx=None, fy=None, fz=None):
         ptrs = [_host_ptr(a, self.npts, n) for a, n in zip((fx, fy, fz), ("fx", "fy", "fz"))]
         self._check(lib().mhd_set_forcing_host(self._h, *ptrs), "mhd_set_forcing_host")
+
+    def get_state(self):
+        """exact-resume blob (spectral state + integrator history + header) as a CUDA uint8 tensor"""
+        torch = _torch()
+        n = int(lib().mhd_state_bytes(self._h))
+        blob = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._before()
+        self._check(lib().mhd_get_state(self._h, _vp(blob.data_ptr()), n), "mhd_get_state")
+        self._after()
+        return blob
+
+    def set_state(self, blob):
+        torch = _torch()
+        if not (isinstance(blob, torch.Tensor) and blob.is_cuda and blob.dtype == torch.uint8 and blob.is_contiguous()):
+            raise ValueError("blob: expected a contiguous CUDA uint8 tensor from get_state()")
+        self._before()
+        self._check(lib().mhd_set_state(self._h, _vp(blob.data_ptr()), int(blob.numel())), "mhd_set_state")
+        self._after()
 
     def step(self, n=1):
         self._check(lib().mhd_step(self._h, int(n)), "mhd_step")
