@@ -55,7 +55,7 @@ def test_batched_3d_and_2d(gpu, ref, shape, batch):
     check(gpu, ref, shape, batch)
 
 
-@pytest.mark.parametrize("n", [256, 512])
+@pytest.mark.parametrize("n", [256, 512, 768])
 def test_round_trip_at_bench_sizes(gpu, n):
     """config 5 sizes the oracle cannot finish in seconds: round trip and Parseval hold at any size."""
     import torch
