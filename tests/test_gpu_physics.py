@@ -86,3 +86,28 @@ def test_orszag_tang_2d_energy_exchange_period(gpu):
     assert abs(T - GOLD["period_2d_orszag_tang"]["value"]) <= 0.08 * GOLD["period_2d_orszag_tang"]["value"], T
     assert abs(T - np.pi) <= 0.03 * np.pi
     assert d["max_divb"] <= 1e-10
+
+
+def test_config2_kelvin_helmholtz_growth_rate_on_the_gpu(gpu):
+    """BASELINE config 2 asks for the linear growth rate: 256^2 hydro KH (profile family of PAPER.md:163-172, eqs 6-7),
+    snapshots every 50 steps; in the linear window t in [0.8, 1.4] the most unstable seeded mode kx = 4
+    (kx a = 0.2, on the rising side of the paper's inverted parabola with its maximum at kx a = 0.4)
+    must grow at the rate of the linear eigen-solve written in tests/test_oracle_kh.py (5 %)."""
+    import torch
+    from test_oracle_kh import amplitude, kh_eig
+    c = inputs.config2(256, 2000)
+    s = gpu.Solver(c.nx, c.ny, c.nz, c.nu, c.eta, c.cs, c.dt, flags=gpu.FLAG_HYDRO)
+    s.set_fields(*[torch.from_numpy(a).cuda() for a in c.arrays()[:4]])
+    s.step(800)
+    ts, amps = [], {k: [] for k in (1, 2, 3, 4)}
+    for i in range(13):
+        uy = s.get_fields()[2][0].cpu().numpy()
+        ts.append((800 + 50 * i) * c.dt)
+        for k in amps:
+            amps[k].append(np.log(amplitude(uy, k)))
+        if i < 12:
+            s.step(50)
+    gam = {k: float(np.polyfit(ts, v, 1)[0]) for k, v in amps.items()}
+    want = kh_eig(256, 0.05, 4, c.nu, c.cs)[0].real
+    assert abs(gam[4] - want) <= 0.05 * want, (gam, want)
+    assert gam[4] > gam[2] > 0.0          # growth increases with kx below the maximum at kx a = 0.4
