@@ -3,6 +3,9 @@
 fp64 MHD timestep wall time and grid-point updates/s at 512^3; HBM GB/s vs peak).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 512]
+    python bench.py --config 1|2|3        # BASELINE configs 1-3 at full length (CUDA-graph replay), oracle timed beside
+    python bench.py --workload fft        # BASELINE config 5 (FFT sweep) alone
+    python bench.py --workload peaks      # measured FP64 / shared-memory ceilings alone
 
 One "step" = one AB2 time step = one pass of the whole hot path over the
 config-4 state (512^3 decaying MHD turbulence, seeded synthetic).  Multi-GPU: the path does not
@@ -75,6 +78,26 @@ def algorithmic_bytes(g, hydro=False):
     b["x_fused"] = (nin + nout) * w2                     # C2R-x + products + R2C-x in one kernel: rows in, rows out
     b["stage"] = (nout + 2 * nin + 2 * nin) * spec       # read flux + state + history, write state + history
     return b
+
+
+def xfused_onchip_model(g, hydro=False):
+    """On-chip work of one x_fused launch that no implementation of this design can avoid:
+    per (z,y) row 4 inverse + 6 forward complex transforms of length nx (two real rows share one), each log8(nx) radix-8
+    passes of nx/8 butterflies: 56 FP64 instructions per butterfly + 28 for the 7 twiddle multiplications of every pass
+    but the first; ~35 FP64 instructions per grid point for the products; between passes every complex (16 B) is written to
+    and read from shared memory once.  Returns (FP64 instruction slots, shared-memory bytes) per launch."""
+    import math
+    nx = g["nx"]
+    rows = g["ny"] * g["nz"]
+    nfft = (2 + 5) if hydro else (4 + 6)
+    passes = max(1, round(math.log(nx, 8)))                 # 512 -> 3 (lengths that are not powers of 8: nearest count)
+    bf = nx // 8
+    dp_fft = bf * (56 * passes + 28 * (passes - 1))
+    dp = rows * (nfft * dp_fft + 35 * nx)
+    smem = rows * (nfft * (passes - 1) * 2 * 16 * nx          # exchanges: store + load of every complex
+                   + (4 if hydro else 7) * 16 * g["nkx"]      # staged input rows read once
+                   + (5 if hydro else 6) * 2 * 16 * g["nkx"])  # Hermitian split: Z[N-k] published and read
+    return dp, smem
 
 
 def survey_reference_bytes(nx, ny, nz):
@@ -210,18 +233,17 @@ def run_gpu(args):
     peak, peak_src = measured_peak()
 
     host = [torch.from_numpy(a).pin_memory() for a in cfg.arrays()]
-    s = mhd.Solver(n, n, n, cfg.nu, cfg.eta, cfg.cs, cfg.dt, device=dev)
+    s = mhd.Solver(n, n, n, cfg.nu, cfg.eta, cfg.cs, cfg.dt, flags=args.flags, device=dev)
     s.set_fields_host(*host)
-    s.step(W)                                       # warm-up (includes the Euler first step)
+    s.step(max(W, 4))                               # warm-up: Euler first step, one eager step, graph capture, first replay
     s.synchronize()
 
-    # ---- timed region: K steps, state resident in HBM (7 fields x 2.3 GB >> 126 MB L2) ----
+    # ---- timed region: K steps on the SHIPPED path (mhd_step = CUDA-graph replay), state resident in HBM ----
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     sampler = ClockSampler(local) if rank == 0 else None
     l0 = mhd.launch_count()
-    s.profile_begin()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(s.stream)
     s.step(K)
@@ -229,34 +251,47 @@ def run_gpu(args):
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
-    prof = s.profile_end()
     launches = mhd.launch_count() - l0
-    clocks = sampler.stop() if sampler else None
     ms_total = max_over_ranks(e0.elapsed_time(e1), dist, dev)
     ms_step = ms_total / K
     value = world * npts * K / (ms_total * 1e-3)
 
+    # ---- second pass, same K steps, eager with a CUDA-event pair around every launch: the per-kernel table ----
+    s.profile_begin()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(s.stream)
+    s.step(K)
+    p1.record(s.stream)
+    torch.cuda.synchronize()
+    prof = s.profile_end()
+    ms_prof_total = p0.elapsed_time(p1)
+
     # ---- end to end through the C ABI with HOST buffers: H2D of the 7 fields, K steps, diagnostics, D2H ----
-    s2 = s
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    s2.set_fields_host(*host)
-    s2.step(K)
-    d = s2.diagnostics(0)
-    s2.get_fields_host(host)
+    s.set_fields_host(*host)
+    s.step(K)
+    d = s.diagnostics(0)
+    s.get_fields_host(host)
     torch.cuda.synchronize()
     e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
+    clocks = sampler.stop() if sampler else None      # sampled from the start of the timed region to the end of the e2e pass
     nfield_bytes = 7 * 8 * npts
     e2e = {"value": world * npts * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nfield_bytes / K,
            "d2h_bytes_per_step": (nfield_bytes + 128) / K,
            "what": f"mhd_set_fields_host (7 pinned fields) + mhd_step({K}) + mhd_diagnostics + mhd_get_fields_host, wall clock"}
+    s.close()
+    del s
 
     if rank != 0:
         return 0
 
-    # ---- roofline of the dominant kernel, timed live with CUDA events inside the timed region ----
+    # ---- measured on-chip ceilings (FP64 FMA pipe, shared-memory data path) for the kernels that are not HBM-bound ----
+    fp64_tflops, smem_gbs = mhd.measure_peaks(dev)
+
+    # ---- per-kernel rooflines, timed live with CUDA events ----
     abytes = algorithmic_bytes(geo)
     traffic = load_traffic()
     kernels = []
@@ -264,27 +299,54 @@ def run_gpu(args):
         if count == 0 or name not in abytes:
             continue
         per = ms / count
-        kernels.append({"kernel": name, "launches_per_step": count / K, "ms_per_launch": per,
-                        "algorithmic_gb": abytes[name] / 1e9, "gbs": abytes[name] / 1e9 / (per * 1e-3),
-                        "frac": abytes[name] / 1e9 / (per * 1e-3) / peak, "share_of_step": ms / ms_total,
-                        "traffic": traffic.get(name)})
+        k = {"kernel": name, "launches_per_step": count / K, "ms_per_launch": per,
+             "algorithmic_gb": abytes[name] / 1e9, "gbs": abytes[name] / 1e9 / (per * 1e-3),
+             "hbm_frac": abytes[name] / 1e9 / (per * 1e-3) / peak, "share_of_step": ms / ms_prof_total,
+             "traffic": traffic.get(name)}
+        floors = {"hbm": abytes[name] / (peak * 1e9) * 1e3}               # ms
+        if name == "x_fused":
+            dp, smem = xfused_onchip_model(geo)
+            floors["alu"] = dp * 2.0 / (fp64_tflops * 1e12) * 1e3          # every FP64 instruction occupies one DFMA slot (2 flop)
+            floors["smem"] = smem / (smem_gbs * 1e9) * 1e3
+            k["fp64_instr"] = dp
+            k["smem_bytes"] = smem
+        k["floors_ms"] = floors
+        k["bound"] = max(floors, key=floors.get)
+        k["frac"] = floors[k["bound"]] / per
+        kernels.append(k)
     kernels.sort(key=lambda k: -k["share_of_step"])
     top = kernels[0]
-    roofline = {"bound": "hbm", "kernel": top["kernel"], "achieved": top["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": top["frac"], "traffic": top["traffic"], "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": abytes[top["kernel"]]}
-    if top["kernel"] == "x_fused":
-        # the whole path is HBM-bound by design and is reported against the HBM roofline; this one kernel is not:
-        roofline["note"] = ("x_fused keeps 7 fields x 8 points per thread in registers (12 warps/SM) and is limited by the FP64 pipe "
-                            "(53 % active) and shared-memory wavefronts (66 %), not by HBM: profiles/r01b_summary.md")
+    unit = {"hbm": "GB/s", "alu": "TFLOP/s", "smem": "GB/s"}[top["bound"]]
+    if top["bound"] == "hbm":
+        achieved, pk, what = top["gbs"], peak, peak_src
+    elif top["bound"] == "alu":
+        achieved, pk = top["fp64_instr"] * 2.0 / 1e12 / (top["ms_per_launch"] * 1e-3), fp64_tflops
+        what = "measured in this run by mhd_measure_peaks (independent DFMA chains; a DFMA slot = 2 flop)"
+    else:
+        achieved, pk = top["smem_bytes"] / 1e9 / (top["ms_per_launch"] * 1e-3), smem_gbs
+        what = "measured in this run by mhd_measure_peaks (conflict-free 16-byte shared-memory stores + loads)"
+    roofline = {"bound": top["bound"], "kernel": top["kernel"], "achieved": achieved, "peak": pk, "unit": unit,
+                "frac": top["frac"], "traffic": top["traffic"], "peak_source": what,
+                "hbm_frac": top["hbm_frac"], "hbm_peak": peak, "hbm_peak_source": peak_src,
+                "algorithmic_bytes_per_launch": abytes[top["kernel"]], "floors_ms": top["floors_ms"],
+                "share_of_step": top["share_of_step"],
+                "note": "bound = the highest of the kernel's floors (HBM bytes, FP64 instruction slots, shared-memory bytes; models in "
+                        "DESIGN.md §6); frac = that floor / measured time; hbm_frac is kept beside it"}
     own_bytes = sum(k["algorithmic_gb"] * 1e9 * k["launches_per_step"] for k in kernels)   # only the kernel classes that ran
     step_roofline = {
         "design_bytes_per_step": own_bytes, "design_gbs": own_bytes / 1e9 / (ms_step * 1e-3),
         "design_frac_of_measured_peak": own_bytes / 1e9 / (ms_step * 1e-3) / peak,
+        "design_frac_of_8TBs": own_bytes / 1e9 / (ms_step * 1e-3) / NOMINAL_HBM_GBS,
         "survey_111F_bytes": survey_reference_bytes(n, n, n),
-        "survey_111F_frac_of_measured_peak": survey_reference_bytes(n, n, n) / 1e9 / peak / (ms_step * 1e-3),
         "survey_111F_frac_of_8TBs": survey_reference_bytes(n, n, n) / 1e9 / NOMINAL_HBM_GBS / (ms_step * 1e-3),
+        "profiled_pass_ms_per_step": ms_prof_total / K,
     }
+
+    # ---- BASELINE metric, second half ("FFT HBM GB/s vs peak"): compact config-5 sweep in the same line ----
+    fft = None
+    if not args.no_fft:
+        torch.cuda.empty_cache()
+        fft = fft_sweep_rows([int(v) for v in args.fft_sizes.split(",")], dev, peak, reps=3, cufft=False)
 
     # ---- the oracle timed beside it on this box's host cores (bounded sample) ----
     cpu = None
@@ -298,29 +360,95 @@ def run_gpu(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"config4: 3D MHD decaying turbulence {n}^3, AB2, 2/3 dealiasing, nu=eta=1e-3, dt=2e-4, cs=1",
                    "grid": [n, n, n], "integrator": "AB2", "multi_gpu": "replicas only (no data-path collective)",
+                   "timed_path": "mhd_step(K): CUDA-graph replay (the shipped path); the per-kernel table comes from a second, eager pass",
                    "l2": "inputs larger than L2 (spectral state 2.2 GB + 18 GB of transients per step vs 126 MB L2)",
-                   "ekin_after_run": d["ekin"], "emag_after_run": d["emag"]},
+                   "flags": args.flags, "ekin_after_run": d["ekin"], "emag_after_run": d["emag"]},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-        "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels, "cpu_baseline": cpu,
+        "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
+        "peaks": {"hbm_gbs": peak, "hbm_source": peak_src, "fp64_tflops": fp64_tflops, "smem_gbs": smem_gbs,
+                  "onchip_source": "mhd_measure_peaks, this run"},
+        "fft": fft, "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
     return 0
 
 
-def run_fft_sweep(args):
-    """--workload fft: BASELINE config 5, batched 3-D R2C + C2R of 7 fields; effective GB/s = 2 F batch / t
-    (input read once + output written once) against the measured copy peak, round-trip error, and cuFFT
-    (torch.fft, never on the product path) as the one permitted reference line."""
+def run_small_config(args):
+    """--config 1|2|3: BASELINE configs 1-3 at their full step count on the shipped path (CUDA-graph replay), AB2, with the
+    oracle timed beside it at FULL length on the host cores.  These grids are L2-resident and launch-bound."""
     import torch
-    from paper_2402_05478_b200 import mhd
+    from paper_2402_05478_b200 import inputs, mhd
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device")
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
-    peak, peak_src = measured_peak()
+    cfg = {1: inputs.config1, 2: inputs.config2, 3: inputs.config3}[args.config]()
+    flags = (mhd.FLAG_HYDRO if cfg.hydro else 0) | args.flags
+    rows = []
+    for integ, name in ((mhd.AB2, "AB2"), (mhd.RK4, "RK4")):
+        s = mhd.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, integrator=integ, flags=flags, device=dev)
+        arrs = [torch.from_numpy(a).to(dev) for a in cfg.arrays()]
+        ts = []
+        l0 = mhd.launch_count()
+        for rep in range(1 + args.reps):
+            s.set_fields(*arrs)
+            s.step(4)                                   # Euler start, eager step, capture, first replay: not timed
+            s.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(s.stream); s.step(cfg.steps); e1.record(s.stream)
+            torch.cuda.synchronize()
+            if rep:
+                ts.append(e0.elapsed_time(e1))
+        ms = statistics.median(ts)
+        d = s.diagnostics(0)
+        rows.append({"integrator": name, "steps": cfg.steps, "ms_per_step": ms / cfg.steps,
+                     "grid_point_updates_per_s": cfg.nx * cfg.ny * cfg.nz * cfg.steps / (ms * 1e-3),
+                     "launches": (mhd.launch_count() - l0) // (1 + args.reps), "ekin": d["ekin"], "emag": d["emag"]})
+        s.close()
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import mhd_ref
+        o = mhd_ref.RefSolver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, flags=1 if cfg.hydro else 0)
+        o.set_fields(*cfg.arrays())
+        t0 = time.perf_counter(); o.step(cfg.steps); sec = time.perf_counter() - t0
+        cpu = {"value": cfg.nx * cfg.ny * cfg.nz * cfg.steps / sec, "unit": UNIT, "cores": mhd_ref.get_threads(), "kind": "oracle",
+               "sample": f"the full config: {cfg.steps} AB2 steps at {cfg.nx}x{cfg.ny}x{cfg.nz}, {sec:.2f} s"}
+        o.close()
+    line = {"metric": METRIC, "value": rows[0]["grid_point_updates_per_s"], "unit": UNIT, "n_gpus": 1, "steps": cfg.steps,
+            "ms_per_step": rows[0]["ms_per_step"], "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {cfg.nx}x{cfg.ny}x{cfg.nz}, {cfg.steps} steps, CUDA-graph replay",
+                       "l2": "L2-resident by construction (the config's whole working set is smaller than L2); launch-bound"},
+            "runs": rows, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_peaks(args):
+    import torch
+    from paper_2402_05478_b200 import mhd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    sampler = ClockSampler(0)
+    vals = [mhd.measure_peaks("cuda:0") for _ in range(3)]
+    clocks = sampler.stop()
+    f, sm = max(v[0] for v in vals), max(v[1] for v in vals)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    mhz = clocks["sm_mhz"] or 0.0
+    line = {"metric": "onchip_peaks", "fp64_tflops": f, "smem_gbs": sm, "clocks": clocks, "sms": sms,
+            "dfma_per_clk_per_sm": (f * 1e12 / 2 / sms / (mhz * 1e6)) if mhz else None,
+            "smem_bytes_per_clk_per_sm": (sm * 1e9 / sms / (mhz * 1e6)) if mhz else None,
+            "hbm_gbs": measured_peak()[0]}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def fft_sweep_rows(sizes, dev, peak, reps=5, cufft=True):
+    """BASELINE config 5: batched 3-D R2C + C2R of 7 fields; effective GB/s = (input + output bytes) / t (the 2F ideal)."""
+    import torch
+    from paper_2402_05478_b200 import mhd
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
-    sweep, l0 = [], mhd.launch_count()
-    for n in [int(v) for v in args.fft_sizes.split(",")]:
+    sweep = []
+    for n in sizes:
         batch = 7
         gen = torch.Generator(device=dev); gen.manual_seed(1005)
         a = torch.rand((batch, n, n, n), dtype=torch.float64, device=dev, generator=gen) * 2.0 - 1.0
@@ -329,7 +457,7 @@ def run_fft_sweep(args):
         back = plan.c2r(spec)
         err = float(torch.linalg.norm(back - a) / torch.linalg.norm(a))
 
-        def timed(fn, reps=5):
+        def timed(fn, reps=reps):
             ts = []
             for it in range(3 + reps):
                 flush.zero_()
@@ -345,16 +473,33 @@ def run_fft_sweep(args):
                "r2c_eff_gbs": (fr + fc) / 1e9 / (t_r2c * 1e-3), "c2r_eff_gbs": (fr + fc) / 1e9 / (t_c2r * 1e-3)}
         row["r2c_frac"] = row["r2c_eff_gbs"] / peak
         row["c2r_frac"] = row["c2r_eff_gbs"] / peak
+        plan.close()
         del plan, back
-        try:   # reference line only: cuFFT through torch.fft
-            t_ref = timed(lambda: torch.fft.rfftn(a, dim=(1, 2, 3)), reps=3)
-            row["cufft_r2c_ms"] = t_ref
-        except Exception as ex:   # out of memory at the largest size is not an error of this library
-            row["cufft_r2c_ms"] = None
-            row["cufft_note"] = type(ex).__name__
+        if cufft:
+            try:   # reference line only: cuFFT through torch.fft
+                row["cufft_r2c_ms"] = timed(lambda: torch.fft.rfftn(a, dim=(1, 2, 3)), reps=3)
+            except Exception as ex:   # out of memory at the largest size is not an error of this library
+                row["cufft_r2c_ms"] = None
+                row["cufft_note"] = type(ex).__name__
         del a, spec
         torch.cuda.empty_cache()
         sweep.append(row)
+    return sweep
+
+
+def run_fft_sweep(args):
+    """--workload fft: BASELINE config 5, batched 3-D R2C + C2R of 7 fields; effective GB/s = 2 F batch / t
+    (input read once + output written once) against the measured copy peak, round-trip error, and cuFFT
+    (torch.fft, never on the product path) as the one permitted reference line."""
+    import torch
+    from paper_2402_05478_b200 import mhd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, peak_src = measured_peak()
+    l0 = mhd.launch_count()
+    sweep = fft_sweep_rows([int(v) for v in args.fft_sizes.split(",")], dev, peak)
     line = {"metric": "fft_effective_gbs", "unit": "GB/s", "n_gpus": 1, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "config5: batched 3-D R2C + C2R, batch 7, uniform[-1,1) reals", "l2": "256 MB flush between iterations"},
             "peak": peak, "peak_source": peak_src, "sweep": sweep, "gpu_launches": mhd.launch_count() - l0,
@@ -390,13 +535,23 @@ def main(argv=None):
     ap.add_argument("--cpu-n", type=int, default=256, help="grid size of the bounded cpu_baseline sample")
     ap.add_argument("--cpu-steps", type=int, default=4, help="timed oracle steps of the cpu_baseline sample (about 10-20 s of CPU work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="step", choices=["step", "fft"], help="step: the 512^3 MHD step (default); fft: the config-5 FFT sweep")
+    ap.add_argument("--workload", default="step", choices=["step", "fft", "peaks"],
+                    help="step: the 512^3 MHD step (default, carries the compact FFT sweep too); fft: the config-5 FFT sweep with the cuFFT line; "
+                         "peaks: the measured FP64 / shared-memory ceilings")
     ap.add_argument("--fft-sizes", default="128,256,512,768")
+    ap.add_argument("--no-fft", action="store_true", help="skip the compact config-5 sweep in the default line")
+    ap.add_argument("--config", type=int, default=0, choices=[0, 1, 2, 3], help="time BASELINE config 1, 2 or 3 at full length instead")
+    ap.add_argument("--reps", type=int, default=3, help="--config: timed repetitions (median)")
+    ap.add_argument("--flags", type=int, default=0, help="extra mhd_create flags (execution-plan switches of include/mhd.h)")
     args = ap.parse_args(argv)
     if args.steps < 1:
         raise SystemExit("--steps must be >= 1")
     if args.impl == "reference":
         return run_reference(args)
+    if args.config:
+        return run_small_config(args)
+    if args.workload == "peaks":
+        return run_peaks(args)
     return run_fft_sweep(args) if args.workload == "fft" else run_gpu(args)
 
 

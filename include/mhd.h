@@ -44,7 +44,14 @@ enum { MHD_AB2 = 0, MHD_RK4 = 1 };
 enum {
     MHD_FLAG_HYDRO = 1u,      /* B == 0 held exactly: induction and Lorentz terms skipped */
     MHD_FLAG_NO_DEALIAS = 2u, /* keep every mode (tests only) */
-    MHD_FLAG_FORCING = 4u     /* reserve workspace for the steady body force f of eq. (2) (mhd_set_forcing) */
+    MHD_FLAG_FORCING = 4u,    /* reserve workspace for the steady body force f of eq. (2) (mhd_set_forcing) */
+    /* Execution-plan switches.  They never change what is computed (results agree to roundoff with the default plan and are
+     * covered by the same parity tests); they exist so that every kernel of the library can be reached, tested and timed
+     * through this ABI.  Nothing in the library reads the environment. */
+    MHD_FLAG_UNFUSED_X = 8u,      /* x C2R, real-space products and x R2C as three kernels through real arrays, instead of the
+                                     fused x pass (the plan that lengths 3*2^a would need if the fused pass did not cover them) */
+    MHD_FLAG_NO_GRAPH = 16u,      /* mhd_step always enqueues its kernels one by one (no CUDA-graph replay) */
+    MHD_FLAG_FUSED_ZSTAGE = 32u   /* last forward FFT axis and the integrator stage in one kernel (the flux spectra are never stored) */
 };
 
 /* mean values are volume averages <.> = (1/N) sum over the grid */
@@ -142,6 +149,9 @@ int  mhd_fft_r2c(mhd_fft_plan* plan, const double* in_real_dev, double* out_comp
 /* inverse, includes 1/(nx*ny*nz); Im of self-conjugate x modes (kx = 0, nx/2 of a row) is ignored */
 int  mhd_fft_c2r(mhd_fft_plan* plan, const double* in_complex_dev, double* out_real_dev);
 void mhd_fft_plan_destroy(mhd_fft_plan* plan);
+const char* mhd_fft_last_error(const mhd_fft_plan* plan);   /* detail of the last MHD_ECUDA on this plan ("" if none) */
+
+/* ==== Instrumentation (not part of the solver's contract; used by bench.py and the tests) ====================== */
 
 /* number of kernel launches this library has enqueued since load (bench.py's gpu_launches) */
 long long mhd_launch_count(void);
@@ -150,12 +160,18 @@ long long mhd_launch_count(void);
  * eagerly with a CUDA-event pair around every launch (on the context's stream); mhd_profile_end
  * synchronises, fills counts[i] (launches) and ms[i] (summed device time) for the
  * mhd_profile_kernel_count() kernel classes named by mhd_profile_kernel_name(i) -- in hot-path
- * order: z inverse, y inverse, x C2R, products, x R2C, fused x pass, y forward, z forward, stage -- and switches
- * profiling off.  Both arrays are HOST memory of that length. */
+ * order: z inverse, y inverse, x C2R, products, x R2C, fused x pass, y forward, z forward, stage, fused z-forward +
+ * stage -- and switches profiling off.  Both arrays are HOST memory of that length. */
 int mhd_profile_kernel_count(void);
 const char* mhd_profile_kernel_name(int i);
 int mhd_profile_begin(mhd_ctx* ctx);
 int mhd_profile_end(mhd_ctx* ctx, int* counts_host, double* ms_host);
+
+/* Measured ceilings of the on-chip resources that bound the fused x pass ("FP64 peak is nominal --
+ * builder to measure"): the FP64 FMA pipe (TFLOP/s, a DFMA = 2 flop, independent register-only chains) and the
+ * shared-memory data path (GB/s moved between shared memory and registers by conflict-free 16-byte accesses).
+ * scratch_dev: DEVICE memory of scratch_bytes >= 4 MiB on the current device; synchronises; results in HOST doubles. */
+int mhd_measure_peaks(void* scratch_dev, size_t scratch_bytes, void* cuda_stream, double* fp64_tflops_host, double* smem_gbs_host);
 
 #ifdef __cplusplus
 }

@@ -54,6 +54,9 @@ struct Layout {
     size_t twx, twy, twz, S, H, Acc, Fh, G, W1, W2, Rf, Rg, red, total;
 };
 
+// the fused x pass keeps real-space data in registers: real arrays are then only staging for set/get/diagnostics/forcing
+bool use_xfuse(int nx, unsigned flags) { return xfused_supported(nx) && !(flags & MHD_FLAG_UNFUSED_X); }
+
 Layout make_layout(const Geometry& g, int integrator, unsigned flags) {
     Layout L;
     size_t o = 0;
@@ -69,7 +72,7 @@ Layout make_layout(const Geometry& g, int integrator, unsigned flags) {
     L.W1 = take(g.nz > 1 ? sizeof(double2) * g.w1field * NPROD : 0);
     L.W2 = take(sizeof(double2) * g.w2field * NPROD);
     L.Rf = take(sizeof(double) * g.npts * NFIELD);
-    L.Rg = take(sizeof(double) * g.npts * NPROD);
+    L.Rg = take(sizeof(double) * g.npts * (use_xfuse(g.nx, flags) ? (int)NFIELD : (int)NPROD));
     L.red = take(sizeof(double) * ((RED_NSUM + 1) * RED_BLOCKS + 64 + 2 * kMaxShell));
     L.total = o;
     return L;
@@ -93,6 +96,7 @@ struct mhd_ctx {
     unsigned flags;
     int hydro;
     cudaStream_t st;
+    int device;                // the device that owns the workspace: every call runs with it current (DeviceGuard)
     char* ws;
     Layout L;
     double2 *twx, *twy, *twz, *S, *H, *Acc, *Fh, *G, *W1, *W2;
@@ -112,6 +116,25 @@ struct mhd_ctx {
 };
 
 namespace {
+
+// Makes `device` current for the duration of one API call and restores the caller's device afterwards, so a context
+// (or plan) created on one GPU can be driven while another GPU is current.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int device) {
+        if (device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = (cudaSetDevice(device) == cudaSuccess);
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+// device that owns a device pointer (-1 if it cannot be determined: the current device is then used as is)
+int owning_device(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return -1; }
+    return (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) ? at.device : -1;
+}
 
 int fail(mhd_ctx* c, int code, const char* what, cudaError_t e = cudaSuccess) {
     if (c) {
@@ -284,8 +307,15 @@ long long mhd_launch_count(void) { return launch_count(); }
 int mhd_profile_kernel_count(void) { return K_NCLASS; }
 const char* mhd_profile_kernel_name(int i) { return (i >= 0 && i < K_NCLASS) ? kClassNames[i] : ""; }
 
+int mhd_measure_peaks(void* scratch, size_t bytes, void* stream, double* fp64_tflops, double* smem_gbs) {
+    if (!scratch || !fp64_tflops || !smem_gbs || bytes < ((size_t)4 << 20)) return MHD_EINVAL;
+    DeviceGuard guard(owning_device(scratch));
+    return measure_peaks((double*)scratch, bytes / sizeof(double), (cudaStream_t)stream, fp64_tflops, smem_gbs) == cudaSuccess ? MHD_OK : MHD_ECUDA;
+}
+
 int mhd_profile_begin(mhd_ctx* c) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     for (int k = 0; k < K_NCLASS; ++k) {
         for (cudaEvent_t ev : c->prof_ev[k]) cudaEventDestroy(ev);
         c->prof_ev[k].clear();
@@ -296,6 +326,7 @@ int mhd_profile_begin(mhd_ctx* c) {
 
 int mhd_profile_end(mhd_ctx* c, int* counts, double* ms) {
     if (!c || !counts || !ms) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     c->profiling = 0;
     CK(cudaStreamSynchronize(c->st));
     for (int k = 0; k < K_NCLASS; ++k) {
@@ -329,7 +360,8 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     if (integrator != MHD_AB2 && integrator != MHD_RK4) return MHD_EINVAL;
     if (!(nu >= 0.0) || !(eta >= 0.0) || !(cs >= 0.0) || !(dt > 0.0)) return MHD_EINVAL;
     if (!isfinite(nu) || !isfinite(eta) || !isfinite(cs) || !isfinite(dt)) return MHD_EINVAL;
-    if (flags & ~(MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS | MHD_FLAG_FORCING)) return MHD_EINVAL;
+    if (flags & ~(MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS | MHD_FLAG_FORCING | MHD_FLAG_UNFUSED_X | MHD_FLAG_NO_GRAPH | MHD_FLAG_FUSED_ZSTAGE))
+        return MHD_EINVAL;
     const Layout L = make_layout(g, integrator, flags);
     if (!workspace || workspace_bytes < L.total || ((size_t)workspace & 255u)) return MHD_EINVAL;
     mhd_ctx* c = new (std::nothrow) mhd_ctx();
@@ -338,10 +370,10 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     c->g = g; c->nu = nu; c->eta = eta; c->cs = cs; c->dt = dt;
     c->integrator = integrator; c->flags = flags; c->hydro = (flags & MHD_FLAG_HYDRO) ? 1 : 0;
     c->st = (cudaStream_t)stream; c->ws = (char*)workspace; c->L = L;
-    c->xfuse = xfused_supported(nx) && getenv("MHD_NO_XFUSE") == nullptr;
-    // z forward pass fused with the stage: correct (parity-tested) but, at one 512-thread CTA per SM, 8 % slower than the two
-    // separate kernels at 512^3 (4.56 vs 4.22 ms, profiles/r01c_zstage.md); opt-in until it wins
-    c->zfuse = nz > 1 && zstage_supported(nz) && getenv("MHD_ZFUSE") != nullptr;
+    c->device = owning_device(workspace);
+    DeviceGuard guard(c->device);
+    c->xfuse = use_xfuse(nx, flags);
+    c->zfuse = nz > 1 && zstage_supported(nz) && (flags & MHD_FLAG_FUSED_ZSTAGE);
     c->prof_ev = new (std::nothrow) std::vector<cudaEvent_t>[K_NCLASS];
     if (!c->prof_ev) { delete c; return MHD_ENOMEM; }
     c->twx = (double2*)(c->ws + L.twx); c->twy = (double2*)(c->ws + L.twy); c->twz = (double2*)(c->ws + L.twz);
@@ -369,6 +401,7 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
 
 void mhd_destroy(mhd_ctx* c) {
     if (!c) return;
+    DeviceGuard guard(c->device);
     if (c->graph) cudaGraphExecDestroy(c->graph);
     if (c->prof_ev) {
         for (int k = 0; k < K_NCLASS; ++k) for (cudaEvent_t ev : c->prof_ev[k]) cudaEventDestroy(ev);
@@ -385,6 +418,7 @@ static void invalidate_graph(mhd_ctx* c) {
 
 int mhd_set_box(mhd_ctx* c, double lx, double ly, double lz) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0) || !isfinite(lx) || !isfinite(ly) || !isfinite(lz))
         return fail(c, MHD_EINVAL, "mhd_set_box: lengths must be finite and > 0");
     const double two_pi = 6.283185307179586476925286766559;
@@ -396,6 +430,7 @@ int mhd_set_box(mhd_ctx* c, double lx, double ly, double lz) {
 
 int mhd_set_forcing(mhd_ctx* c, const double* fx, const double* fy, const double* fz) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!fx && !fy && !fz) { c->have_forcing = 0; invalidate_graph(c); return MHD_OK; }
     if (!fx || !fy || !fz) return fail(c, MHD_EINVAL, "mhd_set_forcing: give all three components or none");
     if (!(c->flags & MHD_FLAG_FORCING)) return fail(c, MHD_ESTATE, "mhd_set_forcing: context created without MHD_FLAG_FORCING");
@@ -412,6 +447,7 @@ int mhd_set_forcing(mhd_ctx* c, const double* fx, const double* fy, const double
 
 int mhd_set_forcing_host(mhd_ctx* c, const double* fx, const double* fy, const double* fz) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!fx && !fy && !fz) return mhd_set_forcing(c, nullptr, nullptr, nullptr);
     if (!fx || !fy || !fz) return fail(c, MHD_EINVAL, "mhd_set_forcing_host: give all three components or none");
     if (!(c->flags & MHD_FLAG_FORCING)) return fail(c, MHD_ESTATE, "mhd_set_forcing_host: context created without MHD_FLAG_FORCING");
@@ -424,6 +460,7 @@ int mhd_set_forcing_host(mhd_ctx* c, const double* fx, const double* fy, const d
 int mhd_set_fields(mhd_ctx* c, const double* rho, const double* ux, const double* uy, const double* uz,
                    const double* bx, const double* by, const double* bz) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_set_fields: NULL field");
     if (!c->hydro && (!bx || !by || !bz)) return fail(c, MHD_EINVAL, "mhd_set_fields: NULL magnetic field without MHD_FLAG_HYDRO");
     const long long n = c->g.npts;
@@ -443,6 +480,7 @@ int mhd_set_fields(mhd_ctx* c, const double* rho, const double* ux, const double
 int mhd_set_fields_host(mhd_ctx* c, const double* rho, const double* ux, const double* uy, const double* uz,
                         const double* bx, const double* by, const double* bz) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_set_fields_host: NULL field");
     if (!c->hydro && (!bx || !by || !bz)) return fail(c, MHD_EINVAL, "mhd_set_fields_host: NULL magnetic field");
     const long long n = c->g.npts;
@@ -457,51 +495,61 @@ int mhd_set_fields_host(mhd_ctx* c, const double* rho, const double* ux, const d
 
 int mhd_step(mhd_ctx* c, int nsteps) {
     if (!c || nsteps < 0) return c ? fail(c, MHD_EINVAL, "mhd_step: nsteps < 0") : MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_step before mhd_set_fields");
     int done = 0;
+    // a launch failure part-way through still leaves `done` completed steps in the state: account for them
+#define CKS(call)                                                                         \
+    do {                                                                                  \
+        cudaError_t e_ = (call);                                                          \
+        if (e_ != cudaSuccess) { c->step += done; return fail(c, MHD_ECUDA, #call, e_); } \
+    } while (0)
     if (nsteps > 0 && c->integrator == MHD_AB2 && !c->have_history) {
-        CK(one_step(c, true));
+        CKS(one_step(c, true));
         c->have_history = 1;
         done = 1;
     }
-    static const bool no_graph = getenv("MHD_NO_GRAPH") != nullptr;
+    const bool no_graph = (c->flags & MHD_FLAG_NO_GRAPH) != 0;
     while (done < nsteps) {
         const int left = nsteps - done;
         if (!no_graph && !c->profiling && c->st != nullptr && (c->graph_ready || left >= 3)) {
             if (!c->graph_ready) {
-                CK(one_step(c, false));   // eager once: sets kernel attributes outside capture
+                CKS(one_step(c, false));   // eager once: sets kernel attributes outside capture
                 ++done;
                 const long long before = launch_count();
                 cudaGraph_t gr = nullptr;
-                CK(cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal));
+                CKS(cudaStreamBeginCapture(c->st, cudaStreamCaptureModeThreadLocal));
                 cudaError_t e = one_step(c, false);
                 cudaError_t e2 = cudaStreamEndCapture(c->st, &gr);
                 if (e != cudaSuccess || e2 != cudaSuccess) {
                     if (gr) cudaGraphDestroy(gr);
+                    c->step += done;
                     return fail(c, MHD_ECUDA, "graph capture", e != cudaSuccess ? e : e2);
                 }
                 c->graph_launches = launch_count() - before;
                 add_launches(-c->graph_launches);   // capture enqueued nothing
                 e = cudaGraphInstantiate(&c->graph, gr, 0);
                 cudaGraphDestroy(gr);
-                if (e != cudaSuccess) return fail(c, MHD_ECUDA, "cudaGraphInstantiate", e);
+                if (e != cudaSuccess) { c->step += done; return fail(c, MHD_ECUDA, "cudaGraphInstantiate", e); }
                 c->graph_ready = 1;
                 continue;
             }
-            CK(cudaGraphLaunch(c->graph, c->st));
+            CKS(cudaGraphLaunch(c->graph, c->st));
             add_launches(c->graph_launches);
             ++done;
         } else {
-            CK(one_step(c, false));
+            CKS(one_step(c, false));
             ++done;
         }
     }
+#undef CKS
     c->step += nsteps;
     return MHD_OK;
 }
 
 int mhd_get_fields(mhd_ctx* c, double* rho, double* ux, double* uy, double* uz, double* bx, double* by, double* bz) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_get_fields: NULL field");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_get_fields before mhd_set_fields");
     const long long n = c->g.npts;
@@ -520,6 +568,7 @@ int mhd_get_fields(mhd_ctx* c, double* rho, double* ux, double* uy, double* uz, 
 
 int mhd_get_fields_host(mhd_ctx* c, double* rho, double* ux, double* uy, double* uz, double* bx, double* by, double* bz) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_get_fields_host: NULL field");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_get_fields_host before mhd_set_fields");
     const long long n = c->g.npts;
@@ -558,6 +607,7 @@ size_t mhd_state_bytes(const mhd_ctx* c) {
 
 int mhd_get_state(mhd_ctx* c, void* state, size_t bytes) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!state || bytes < mhd_state_bytes(c)) return fail(c, MHD_EINVAL, "mhd_get_state: buffer missing or too small");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_get_state before mhd_set_fields");
     StateHeader h;
@@ -577,6 +627,7 @@ int mhd_get_state(mhd_ctx* c, void* state, size_t bytes) {
 
 int mhd_set_state(mhd_ctx* c, const void* state, size_t bytes) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!state || bytes < mhd_state_bytes(c)) return fail(c, MHD_EINVAL, "mhd_set_state: buffer missing or too small");
     StateHeader h;
     CK(cudaMemcpyAsync(&h, state, sizeof(h), cudaMemcpyDeviceToHost, c->st));
@@ -594,16 +645,17 @@ int mhd_set_state(mhd_ctx* c, const void* state, size_t bytes) {
 
 int mhd_diagnostics(mhd_ctx* c, mhd_diag* out, double* ekin_spec, double* emag_spec, int nshell) {
     if (!c) return MHD_EINVAL;
+    DeviceGuard guard(c->device);
     if (!out || nshell < 0 || nshell > kMaxShell || (nshell > 0 && (!ekin_spec || !emag_spec)))
         return fail(c, MHD_EINVAL, "mhd_diagnostics: bad argument");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_diagnostics before mhd_set_fields");
     const Geometry& g = c->g;
     const long long n = g.npts;
     const SpecGeom sg = spec_geom(g);
-    CK(inverse_fields(c, c->S, c->hydro ? 4 : NFIELD, c->Rf));
-    CK(launch_reduce_fields(c->Rf, n, c->hydro, c->red_partial, c->red_result, c->st));
     if (nshell > 0 && (c->kf[0] != 1.0 || c->kf[1] != 1.0 || (g.nz > 1 && c->kf[2] != 1.0)))
         return fail(c, MHD_EINVAL, "mhd_diagnostics: shell spectra are defined on the 2*pi box only");
+    CK(inverse_fields(c, c->S, c->hydro ? 4 : NFIELD, c->Rf));
+    CK(launch_reduce_fields(c->Rf, n, c->hydro, c->red_partial, c->red_result, c->st));
     {
         // Velocity spectrum and the paper's diagnostics (Omega(t), Rayleigh quotient): u = m/rho is not band-limited, and the spectrum is defined over ALL modes
         // (it sums to 1/2 <|u|^2>), so u^ comes from an unpruned forward transform:
@@ -673,20 +725,59 @@ int mhd_diagnostics(mhd_ctx* c, mhd_diag* out, double* ekin_spec, double* emag_s
 struct mhd_fft_plan {
     int nx, ny, nz, batch, nxh;
     cudaStream_t st;
+    int device;
     double2 *twx, *twy, *twz, *work;
+    int plane;                 // x and y passes fused per plane through L2 (planefft_kernel.cu)
+    int group, ring_slots, lag, pitch;
+    double2* ring;
+    unsigned* counters;
+    char err[256];
 };
 
 namespace {
-struct FftLayout { size_t twx, twy, twz, work, total; };
+// plane pipeline geometry: groups of about 4 MB (>= 64 x-row items per group), the x pass 3 groups ahead of the y pass
+#ifndef MHD_PF_LAG
+#define MHD_PF_LAG 3
+#endif
+#ifndef MHD_PF_MINITEMS
+#define MHD_PF_MINITEMS 64
+#endif
+struct PlaneGeom { int group, ring_slots, lag, pitch; };
+PlaneGeom plane_geom(int n) {
+    PlaneGeom g;
+    const int tp = n / 8, teams = 512 / tp;
+    const int per_plane = (n / 2 + teams - 1) / teams;
+    g.group = (MHD_PF_MINITEMS + per_plane - 1) / per_plane;
+    g.lag = MHD_PF_LAG;
+    g.ring_slots = g.lag + 2;
+    g.pitch = (n / 2 + 1 + 7) / 8 * 8;
+    return g;
+}
+struct FftLayout { size_t twx, twy, twz, work, ring, counters, total; };
 FftLayout make_fft_layout(int nx, int ny, int nz, int batch) {
     FftLayout L;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
     L.twx = take(sizeof(double2) * nx); L.twy = take(sizeof(double2) * ny); L.twz = take(sizeof(double2) * nz);
     L.work = take(sizeof(double2) * (size_t)(nx / 2 + 1) * ny * nz * batch);
+    L.ring = L.counters = o;
+    if (planefft_supported(nx, ny)) {
+        const PlaneGeom g = plane_geom(nx);
+        L.ring = take(sizeof(double2) * (size_t)g.ring_slots * g.group * ny * g.pitch);
+        L.counters = take(planefft_counter_bytes((long long)batch * nz, g.group));
+    }
     L.total = o;
     return L;
 }
+int pfail(mhd_fft_plan* p, const char* what, cudaError_t e) {
+    snprintf(p->err, sizeof(p->err), "%s: %s", what, cudaGetErrorString(e));
+    return MHD_ECUDA;
+}
+#define PCK(call)                                            \
+    do {                                                     \
+        cudaError_t e_ = (call);                             \
+        if (e_ != cudaSuccess) return pfail(p, #call, e_);   \
+    } while (0)
 bool fft_dims_ok(int nx, int ny, int nz, int batch) {
     return fft_size_supported(nx) && fft_size_supported(ny) && (nz == 1 || fft_size_supported(nz)) && batch >= 1 && batch <= 4096;
 }
@@ -707,9 +798,18 @@ int mhd_fft_plan_create(mhd_fft_plan** out, int nx, int ny, int nz, int batch, v
     if (!workspace || bytes < L.total || ((size_t)workspace & 255u)) return MHD_EINVAL;
     mhd_fft_plan* p = new (std::nothrow) mhd_fft_plan();
     if (!p) return MHD_ENOMEM;
+    p->err[0] = 0;
+    p->device = owning_device(workspace);
+    DeviceGuard guard(p->device);
     p->nx = nx; p->ny = ny; p->nz = nz; p->batch = batch; p->nxh = nx / 2 + 1; p->st = (cudaStream_t)stream;
     char* ws = (char*)workspace;
     p->twx = (double2*)(ws + L.twx); p->twy = (double2*)(ws + L.twy); p->twz = (double2*)(ws + L.twz); p->work = (double2*)(ws + L.work);
+    p->plane = planefft_supported(nx, ny) ? 1 : 0;
+    if (p->plane) {
+        const PlaneGeom g = plane_geom(nx);
+        p->group = g.group; p->ring_slots = g.ring_slots; p->lag = g.lag; p->pitch = g.pitch;
+        p->ring = (double2*)(ws + L.ring); p->counters = (unsigned*)(ws + L.counters);
+    }
     std::vector<double2> t;
     const int n3[3] = {nx, ny, nz};
     double2* d3[3] = {p->twx, p->twy, p->twz};
@@ -726,28 +826,42 @@ int mhd_fft_plan_create(mhd_fft_plan** out, int nx, int ny, int nz, int batch, v
 
 void mhd_fft_plan_destroy(mhd_fft_plan* p) { delete p; }
 
+const char* mhd_fft_last_error(const mhd_fft_plan* p) { return p ? p->err : ""; }
+
 int mhd_fft_r2c(mhd_fft_plan* p, const double* in, double* out) {
     if (!p || !in || !out) return MHD_EINVAL;
+    DeviceGuard guard(p->device);
     double2* o = (double2*)out;
     const long long plane = (long long)p->ny * p->nxh, vol = plane * p->nz;
-    RowArgs r;
-    r.spec = o; r.real = const_cast<double*>(in); r.spec_pitch = p->nxh; r.real_pitch = p->nx;
-    r.nrows = (long long)p->batch * p->nz * p->ny; r.nkx = p->nxh; r.scale = 1.0;
-    if (launch_fft_rows(p->nx, false, r, p->twx, p->st) != cudaSuccess) return MHD_ECUDA;
     AxisArgs a;
-    a.in = o; a.out = o; a.nouter = (long long)p->batch * p->nz; a.in_outer = a.out_outer = plane;
-    a.in_row = a.out_row = p->nxh; a.inner = p->nxh; a.nk_in = a.nk_out = p->ny; a.scale = 1.0;
-    if (launch_fft_axis(p->ny, false, a, p->twy, p->st) != cudaSuccess) return MHD_ECUDA;
+    a.scale = 1.0;
+    if (p->plane) {   // x and y in one persistent kernel, plane by plane through L2: the x-transformed rows never reach HBM
+        PlaneFftArgs f;
+        f.real = const_cast<double*>(in); f.spec_in = nullptr; f.spec_out = o; f.ring = p->ring; f.counters = p->counters;
+        f.nplanes = (long long)p->batch * p->nz; f.group = p->group; f.ngroups = (f.nplanes + f.group - 1) / f.group;
+        f.nxh = p->nxh; f.pitch = p->pitch; f.ring_slots = p->ring_slots; f.lag = p->lag; f.scale = 1.0;
+        PCK(launch_planefft(p->nx, false, f, p->twx, p->st));
+    } else {
+        RowArgs r;
+        r.spec = o; r.real = const_cast<double*>(in); r.spec_pitch = p->nxh; r.real_pitch = p->nx;
+        r.nrows = (long long)p->batch * p->nz * p->ny; r.nkx = p->nxh; r.scale = 1.0;
+        PCK(launch_fft_rows(p->nx, false, r, p->twx, p->st));
+        a.in = o; a.out = o; a.nouter = (long long)p->batch * p->nz; a.in_outer = a.out_outer = plane;
+        a.in_row = a.out_row = p->nxh; a.inner = p->nxh; a.nk_in = a.nk_out = p->ny;
+        PCK(launch_fft_axis(p->ny, false, a, p->twy, p->st));
+    }
+    a.in = o; a.out = o;
     if (p->nz > 1) {
         a.nouter = p->batch; a.in_outer = a.out_outer = vol; a.in_row = a.out_row = plane;
         a.inner = (int)plane; a.nk_in = a.nk_out = p->nz;
-        if (launch_fft_axis(p->nz, false, a, p->twz, p->st) != cudaSuccess) return MHD_ECUDA;
+        PCK(launch_fft_axis(p->nz, false, a, p->twz, p->st));
     }
     return MHD_OK;
 }
 
 int mhd_fft_c2r(mhd_fft_plan* p, const double* in, double* out) {
     if (!p || !in || !out) return MHD_EINVAL;
+    DeviceGuard guard(p->device);
     const double2* src = (const double2*)in;
     const long long plane = (long long)p->ny * p->nxh, vol = plane * p->nz;
     AxisArgs a;
@@ -755,17 +869,26 @@ int mhd_fft_c2r(mhd_fft_plan* p, const double* in, double* out) {
     if (p->nz > 1) {
         a.in = src; a.out = p->work; a.nouter = p->batch; a.in_outer = a.out_outer = vol; a.in_row = a.out_row = plane;
         a.inner = (int)plane; a.nk_in = a.nk_out = p->nz;
-        if (launch_fft_axis(p->nz, true, a, p->twz, p->st) != cudaSuccess) return MHD_ECUDA;
+        PCK(launch_fft_axis(p->nz, true, a, p->twz, p->st));
         src = p->work;
+    }
+    if (p->plane) {   // y and x in one persistent kernel, plane by plane through L2
+        PlaneFftArgs f;
+        f.real = out; f.spec_in = src; f.spec_out = nullptr; f.ring = p->ring; f.counters = p->counters;
+        f.nplanes = (long long)p->batch * p->nz; f.group = p->group; f.ngroups = (f.nplanes + f.group - 1) / f.group;
+        f.nxh = p->nxh; f.pitch = p->pitch; f.ring_slots = p->ring_slots; f.lag = p->lag;
+        f.scale = 1.0 / ((double)p->nx * (double)p->ny * (double)p->nz);
+        PCK(launch_planefft(p->nx, true, f, p->twx, p->st));
+        return MHD_OK;
     }
     a.in = src; a.out = p->work; a.nouter = (long long)p->batch * p->nz; a.in_outer = a.out_outer = plane;
     a.in_row = a.out_row = p->nxh; a.inner = p->nxh; a.nk_in = a.nk_out = p->ny;
-    if (launch_fft_axis(p->ny, true, a, p->twy, p->st) != cudaSuccess) return MHD_ECUDA;
+    PCK(launch_fft_axis(p->ny, true, a, p->twy, p->st));
     RowArgs r;
     r.spec = p->work; r.real = out; r.spec_pitch = p->nxh; r.real_pitch = p->nx;
     r.nrows = (long long)p->batch * p->nz * p->ny; r.nkx = p->nxh;
     r.scale = 1.0 / ((double)p->nx * (double)p->ny * (double)p->nz);
-    if (launch_fft_rows(p->nx, true, r, p->twx, p->st) != cudaSuccess) return MHD_ECUDA;
+    PCK(launch_fft_rows(p->nx, true, r, p->twx, p->st));
     return MHD_OK;
 }
 

@@ -30,6 +30,22 @@ bool fft_size_supported(int n);
 cudaError_t launch_fft_axis(int n, bool inverse, const AxisArgs& a, const double2* tw, cudaStream_t st);
 cudaError_t launch_fft_rows(int n, bool inverse, const RowArgs& a, const double2* tw, cudaStream_t st);
 
+// ---- x and y passes of a batched 3-D real FFT in one persistent kernel, plane by plane through L2 (planefft_kernel.cu) ----
+struct PlaneFftArgs {
+    double* real;             // [nplanes][n][n] doubles: input (forward) or output (inverse)
+    const double2* spec_in;   // inverse: [nplanes][n][nxh] half-spectrum planes (y not yet transformed)
+    double2* spec_out;        // forward: [nplanes][n][nxh] half-spectrum planes (x and y transformed)
+    double2* ring;            // ring_slots * group planes of n * pitch complex (the L2-resident intermediate)
+    unsigned* counters;       // planefft_counter_bytes(...) bytes, 8-byte aligned; zeroed by the launcher
+    long long nplanes, ngroups;
+    int nxh, pitch;           // n/2+1 and the ring's row pitch (multiple of 8)
+    int group, ring_slots, lag;
+    double scale;             // applied by the inverse x pass
+};
+bool planefft_supported(int nx, int ny);
+size_t planefft_counter_bytes(long long nplanes, int group);
+cudaError_t launch_planefft(int n, bool inverse, const PlaneFftArgs& a, const double2* tw, cudaStream_t st);
+
 // ---- fused x pass (xfused_kernel.cu): C2R-x -> products -> R2C-x, in place on [field][row][px] ----
 struct XFusedArgs {
     double2* w2;              // inputs: fields 0..6 (0..3 hydro); outputs: product fields 0..11 (0..8 hydro)
@@ -103,5 +119,21 @@ cudaError_t launch_spectrum(const SpecGeom& g, const double2* V3, double* rowbin
 void count_launch();
 long long launch_count();
 void add_launches(long long n);
+
+// ---- instrumentation: measured FP64-FMA and shared-memory ceilings (peaks_kernel.cu) ----
+cudaError_t measure_peaks(double* scratch, size_t scratch_doubles, cudaStream_t st, double* fp64_tflops, double* smem_gbs);
+
+// ---- per-device one-time kernel setup ---------------------------------------------------------------
+// cudaFuncSetAttribute (opt-in dynamic shared memory) and the SM count belong to a DEVICE, not to the process: every
+// launcher keeps one DeviceOnce per kernel family and asks it for the current device's slot.
+constexpr int kMaxDevices = 64;
+struct DeviceOnce {
+    bool done[kMaxDevices];
+    int sms[kMaxDevices];
+};
+// index of the calling thread's current device in a DeviceOnce (cudaGetDevice), or -1 on error / out of range
+int device_slot();
+// SM count of device slot `dev` (cached per device)
+cudaError_t device_sm_count(int dev, int* sms);
 
 }  // namespace mhd

@@ -11,6 +11,24 @@ void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 long long launch_count() { return g_launches.load(std::memory_order_relaxed); }
 void add_launches(long long n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+int device_slot() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
+    return dev;
+}
+cudaError_t device_sm_count(int dev, int* sms) {
+    static int cache[kMaxDevices];           // 0 = not asked yet (benign race: every writer stores the same value)
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    if (cache[dev] == 0) {
+        int v = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        cache[dev] = v;
+    }
+    *sms = cache[dev];
+    return cudaSuccess;
+}
+
 static constexpr int kThreads = 256;
 static constexpr int kGridStream = 148 * 8;   // grid-stride kernels: 8 CTAs of 256 threads per SM
 

@@ -1,0 +1,84 @@
+// peaks_kernel.cu — measured ceilings of the two on-chip resources that bound the fused x pass (instrumentation, not on the
+// solver's path): the FP64 FMA pipe and the shared-memory data path.  SURVEY.md §8(d) leaves the FP64 peak "nominal —
+// builder to measure"; bench.py --workload peaks (and the default bench line) report x_fused against these numbers.
+//
+//   fp64 : every thread runs 8 independent DFMA chains (x = x*a + b), 148*k CTAs of 256 threads, no memory traffic.
+//          flops = 2 per DFMA.
+//   smem : every thread alternates conflict-free STS.128 / LDS.128 on its own 16-byte slot pattern (a warp moves 512 B =
+//          4 wavefronts of 128 B per instruction).  bytes = 16 per thread per instruction.
+#include "mhd_internal.h"
+
+namespace mhd {
+
+__global__ void __launch_bounds__(256) peak_fp64_kernel(double* __restrict__ out, int iters, double a, double b) {
+    double x0 = threadIdx.x * 1e-3, x1 = x0 + 1.0, x2 = x0 + 2.0, x3 = x0 + 3.0, x4 = x0 + 4.0, x5 = x0 + 5.0, x6 = x0 + 6.0, x7 = x0 + 7.0;
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+__global__ void __launch_bounds__(256) peak_smem_kernel(double* __restrict__ out, int iters) {
+    __shared__ double2 sm[4 * 256];
+    double2 v0 = make_double2(threadIdx.x, 1.0), v1 = make_double2(2.0, threadIdx.x), v2 = v0, v3 = v1;
+    double2* p = sm + threadIdx.x;              // consecutive lanes -> consecutive 16-byte slots: conflict-free
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+        p[0] = v0; p[256] = v1; p[512] = v2; p[768] = v3;
+        __syncwarp();
+        const int o = (it & 1) ? 1 : 31;        // read a neighbour's slot of the same warp so nothing is forwarded in registers
+        const double2* q = sm + (threadIdx.x & ~31) + ((threadIdx.x + o) & 31);
+        v0 = q[0]; v1 = q[256]; v2 = q[512]; v3 = q[768];
+        __syncwarp();
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = v0.x + v1.y + v2.x + v3.y;
+}
+
+// scratch: >= grid*256 doubles.  Best of `reps` launches each; results in TFLOP/s and GB/s.
+cudaError_t measure_peaks(double* scratch, size_t scratch_doubles, cudaStream_t st, double* fp64_tflops, double* smem_gbs) {
+    const int dev = device_slot();
+    int sms = 0;
+    cudaError_t e = device_sm_count(dev, &sms);
+    if (e != cudaSuccess) return e;
+    const int grid = sms * 8;                   // 8 CTAs of 256 threads per SM: 64 warps per SM
+    if (scratch_doubles < (size_t)grid * 256) return cudaErrorInvalidValue;
+    cudaEvent_t a, b;
+    if ((e = cudaEventCreate(&a)) != cudaSuccess) return e;
+    if ((e = cudaEventCreate(&b)) != cudaSuccess) { cudaEventDestroy(a); return e; }
+    const int reps = 5;
+    double best_f = 0.0, best_s = 0.0;
+    for (int r = 0; r < reps + 1 && e == cudaSuccess; ++r) {
+        const int iters = 4096;
+        cudaEventRecord(a, st);
+        peak_fp64_kernel<<<grid, 256, 0, st>>>(scratch, iters, 0.999999, 1e-9);
+        count_launch();
+        cudaEventRecord(b, st);
+        if ((e = cudaEventSynchronize(b)) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        const double flops = 2.0 * 8.0 * 16.0 * (double)iters * 256.0 * (double)grid;
+        if (r > 0 && ms > 0.f) best_f = fmax(best_f, flops / (ms * 1e-3) / 1e12);
+        const int it2 = 8192;
+        cudaEventRecord(a, st);
+        peak_smem_kernel<<<grid, 256, 0, st>>>(scratch, it2);
+        count_launch();
+        cudaEventRecord(b, st);
+        if ((e = cudaEventSynchronize(b)) != cudaSuccess) break;
+        cudaEventElapsedTime(&ms, a, b);
+        const double bytes = 16.0 * 8.0 * (double)it2 * 256.0 * (double)grid;      // 4 stores + 4 loads of 16 B per iteration
+        if (r > 0 && ms > 0.f) best_s = fmax(best_s, bytes / (ms * 1e-3) / 1e9);
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    *fp64_tflops = best_f;
+    *smem_gbs = best_s;
+    return e;
+}
+
+}  // namespace mhd

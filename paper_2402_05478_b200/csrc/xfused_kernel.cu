@@ -27,118 +27,17 @@
 // HBM traffic: reads 7 rows of nkx complex, writes 12 rows of nkx complex, in place in the same
 // [field][row][px] array (a row's inputs are all consumed before its outputs are written).
 #include "mhd_internal.h"
-#include "fft_core.cuh"
+#include "xteam.cuh"
 
 #ifndef MHD_XF_PREFETCH
 #define MHD_XF_PREFETCH 1
 #endif
-// threads per persistent CTA for N >= 256 (a multiple of 128): 384 = 6 rows in flight per SM at N = 512
-// twiddles w^2..w^7 of a radix-8 pass by multiplication from w: 0 = never (7 table reads), 1 = last pass, 2 = every pass.
-// The kernel is bound by shared-memory wavefronts (80 % of the LSU data pipe), not FP64 (43 %): 2 is fastest (B200, 512^3).
-#ifndef MHD_XF_TWCHAIN
-#define MHD_XF_TWCHAIN 2
-#endif
-#ifndef MHD_XF_THREADS
-#define MHD_XF_THREADS 384
-#endif
+// MHD_XF_THREADS (xteam.cuh): threads per persistent CTA for N >= 256 (a multiple of 128): 384 = 6 rows in flight per SM at N = 512
+// MHD_XF_TWCHAIN (xteam.cuh): the kernel is bound by shared-memory wavefronts (80 % of the LSU data pipe), not FP64 (43 %): 2 is
+// fastest (B200, 512^3).
 
 namespace mhd {
 using namespace mhdfft;
-
-template <int N> struct XCfg {
-    static constexpr int TP = Plan<N>::TP;                      // threads per row
-    static constexpr int THREADS = (N >= 256) ? (MHD_XF_THREADS / TP) * TP : 128;   // whole teams only
-    static constexpr int TEAMS = THREADS / TP;                  // rows in flight per CTA
-    static constexpr int BUF = Padded::size(N);                 // complex elements per exchange buffer
-    // number of twiddle-table entries: sum over passes s >= 1 of (R_s - 1) * P_s
-    __host__ __device__ static constexpr int tw_offset(int s) {  // first entry of pass s
-        int off = 0, P = Plan<N>::radix(0);
-        for (int t = 1; t < s; ++t) { off += (Plan<N>::radix(t) - 1) * P; P *= Plan<N>::radix(t); }
-        return off;
-    }
-    static constexpr int NTW = tw_offset(Plan<N>::NP);
-    static constexpr size_t SMEM = sizeof(cplx) * ((size_t)2 * BUF * TEAMS + (NTW > 0 ? NTW : 1));
-};
-
-template <int TP> __device__ __forceinline__ void team_sync(int team) {
-    if constexpr (TP >= 64) asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "n"(TP) : "memory");
-    else __syncwarp();
-}
-
-__device__ __forceinline__ constexpr int xpad(int e) { return e + (e >> 3); }
-// padded index of (e + D) for a compile-time D, given e and xpad(e)
-template <int D> __device__ __forceinline__ int xpad_add(int e, int pe) {
-    if constexpr (D % 8 == 0) return pe + D + D / 8;
-    else return xpad(e + D);
-}
-
-// One Stockham pass S (P = product of the radices done) on the 8 register values of slot i; the
-// exchange before the next pass goes through sm0 (the following one through sm1, and so on).
-template <int N, bool INV, int S, int P>
-struct XPass {
-    using PL = Plan<N>;
-    static constexpr int R = PL::radix(S);
-    static constexpr int E = PL::E;
-    static constexpr int TP = PL::TP;
-    static constexpr bool LAST = (S == PL::NP - 1);
-    __device__ __forceinline__ static void run(cplx (&v)[E], cplx* sm0, cplx* sm1, int i, int team, const cplx* __restrict__ stw) {
-#pragma unroll
-        for (int m = 0; m < E / R; ++m) {
-            const int b = i + TP * m;
-            const int k = b & (P - 1);
-            if constexpr (S > 0) {
-                const cplx* __restrict__ t = stw + XCfg<N>::tw_offset(S) + k;
-                if constexpr (R == 8 && (MHD_XF_TWCHAIN >= 2 || (MHD_XF_TWCHAIN == 1 && P >= 32))) {
-                    // the kernel is bound by shared-memory wavefronts, not FP64: read w and form w^2..w^7 by
-                    // multiplication (depth <= 3, a few ulp) instead of 7 conflict-free but 4-wavefront reads
-                    cplx w1 = t[0];
-                    if (INV) w1.y = -w1.y;
-                    const cplx w2 = cmul(w1, w1), w3 = cmul(w2, w1), w4 = cmul(w2, w2);
-                    const cplx w5 = cmul(w4, w1), w6 = cmul(w3, w3), w7 = cmul(w4, w3);
-                    v[m * R + 1] = cmul(v[m * R + 1], w1); v[m * R + 2] = cmul(v[m * R + 2], w2);
-                    v[m * R + 3] = cmul(v[m * R + 3], w3); v[m * R + 4] = cmul(v[m * R + 4], w4);
-                    v[m * R + 5] = cmul(v[m * R + 5], w5); v[m * R + 6] = cmul(v[m * R + 6], w6);
-                    v[m * R + 7] = cmul(v[m * R + 7], w7);
-                } else {
-#pragma unroll
-                    for (int q = 1; q < R; ++q) {
-                        cplx w = t[(q - 1) * P];
-                        if (INV) w.y = -w.y;
-                        v[m * R + q] = cmul(v[m * R + q], w);
-                    }
-                }
-            }
-            bfly<R, INV>(&v[m * R]);
-            if constexpr (!LAST) {
-                if constexpr (P == 1) {            // first pass: j = R*b, element j + q
-                    const int j = b * R, pj = xpad(j);
-#pragma unroll
-                    for (int q = 0; q < R; ++q) sm0[(R == 8) ? pj + q : xpad(j + q)] = v[m * R + q];
-                } else {
-                    const int j = (b - k) * R + k, pj = xpad(j);
-#pragma unroll
-                    for (int q = 0; q < R; ++q) sm0[(P % 8 == 0) ? pj + q * (P + P / 8) : xpad(j + q * P)] = v[m * R + q];
-                }
-            }
-        }
-        if constexpr (!LAST) {
-            constexpr int Rn = PL::radix(S + 1);
-            team_sync<TP>(team);
-            const int pi = xpad(i);
-#pragma unroll
-            for (int m = 0; m < E / Rn; ++m)
-#pragma unroll
-                for (int q = 0; q < Rn; ++q) {
-                    const int D = TP * m + q * (N / Rn);
-                    v[m * Rn + q] = sm0[(D % 8 == 0) ? pi + D + D / 8 : xpad(i + D)];
-                }
-            XPass<N, INV, S + 1, P * R>::run(v, sm1, sm0, i, team, stw);
-        }
-    }
-};
-
-// number of exchanges of one transform (decides which buffer the next exchange uses)
-template <int N> __device__ __forceinline__ constexpr bool odd_exchanges() { return ((Plan<N>::NP - 1) & 1) != 0; }
 
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
@@ -520,19 +419,143 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
     }
 }
 
+// Lengths 3*2^a (12 or 24 points per thread, a radix-3 last pass): the same team machinery with one exchange buffer per
+// team and general first/last-pass index sets.  128 threads per CTA (4 teams at N = 768), persistent.
+template <int N> struct XRowGenCfg {
+    static constexpr int TP = Plan<N>::TP;
+    static constexpr int THREADS = 128;
+    static constexpr int TEAMS = THREADS / TP;
+    static constexpr size_t SMEM = sizeof(cplx) * ((size_t)XCfg<N>::BUF * TEAMS + (XCfg<N>::NTW > 0 ? XCfg<N>::NTW : 1));
+};
+
+template <int N, bool INV>
+__global__ void __launch_bounds__(XRowGenCfg<N>::THREADS, 3) xrows_general_kernel(RowArgs a, const cplx* __restrict__ tw) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    using PL = Plan<N>;
+    using CF = XCfg<N>;
+    using RC = XRowGenCfg<N>;
+    constexpr int TP = PL::TP, E = PL::E;
+    constexpr int R0 = PL::radix(0), RL = PL::radix(PL::NP - 1);
+    const int team = threadIdx.x / TP, i = threadIdx.x % TP;
+    cplx* const smbase = reinterpret_cast<cplx*>(smraw);
+    cplx* const stw = smbase + (size_t)CF::BUF * RC::TEAMS;
+    cplx* const buf = smbase + (size_t)team * CF::BUF;
+    const int nkx = a.nkx;
+    {
+        int P = PL::radix(0);
+#pragma unroll
+        for (int s = 1; s < PL::NP; ++s) {
+            const int R = PL::radix(s), off = CF::tw_offset(s);
+            for (int e = threadIdx.x; e < (R - 1) * P; e += blockDim.x) {
+                const int q = e / P + 1, k = e % P;
+                stw[off + e] = tw[k * q * (N / (P * R))];
+            }
+            P *= R;
+        }
+    }
+    __syncthreads();
+    const long long npairs = (a.nrows + 1) / 2;
+    const long long stride = (long long)gridDim.x * RC::TEAMS;
+    for (long long pr = (long long)blockIdx.x * RC::TEAMS + team; pr - team < npairs; pr += stride) {
+        const bool ok = pr < npairs;
+        const long long r0 = ok ? 2 * pr : 0;
+        cplx* __restrict__ A = a.spec + r0 * a.spec_pitch;
+        cplx* __restrict__ B = A + a.spec_pitch;
+        double* __restrict__ ra = a.real + r0 * a.real_pitch;
+        double* __restrict__ rb = ra + a.real_pitch;
+        cplx v[E];
+        if constexpr (INV) {
+#pragma unroll
+            for (int m = 0; m < E / R0; ++m)
+#pragma unroll
+                for (int q = 0; q < R0; ++q) {
+                    const int k = first_index<N>(i, m, q);
+                    const bool lo = k < nkx, hi = (N - k) < nkx;
+                    const int idx = lo ? k : N - k;
+                    cplx x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
+                    if (ok && (lo || hi)) { x = A[idx]; y = B[idx]; }
+                    if (k == 0 || 2 * k == N) { x.y = 0.0; y.y = 0.0; }                 // self-conjugate modes: Im ignored
+                    v[first_reg<N>(m, q)] = lo ? make_double2(x.x - y.y, x.y + y.x) : make_double2(x.x + y.y, y.x - x.y);
+                }
+            XPass<N, true, 0, 1, true>::run(v, buf, buf, i, team, stw);
+            const double s = a.scale;
+            if (ok) {
+#pragma unroll
+                for (int m = 0; m < E / RL; ++m)
+#pragma unroll
+                    for (int q = 0; q < RL; ++q) {
+                        const int x = last_index<N>(i, m, q);
+                        ra[x] = v[last_reg<N>(m, q)].x * s;
+                        rb[x] = v[last_reg<N>(m, q)].y * s;
+                    }
+            }
+        } else {
+#pragma unroll
+            for (int m = 0; m < E / R0; ++m)
+#pragma unroll
+                for (int q = 0; q < R0; ++q) {
+                    const int x = first_index<N>(i, m, q);
+                    v[first_reg<N>(m, q)] = ok ? make_double2(ra[x], rb[x]) : make_double2(0.0, 0.0);
+                }
+            XPass<N, false, 0, 1, true>::run(v, buf, buf, i, team, stw);
+            // Hermitian split: publish Z[j] for the j some k = N - j < nkx will ask for, at position N - j (unpadded)
+#pragma unroll
+            for (int m = 0; m < E / RL; ++m)
+#pragma unroll
+                for (int q = 0; q < RL; ++q) {
+                    const int j = last_index<N>(i, m, q);
+                    if (j >= 1 && N - j < nkx) buf[N - j] = v[last_reg<N>(m, q)];
+                }
+            team_sync<TP>(team);
+            const double s = 0.5 * a.scale;
+            if (ok) {
+#pragma unroll
+                for (int m = 0; m < E / RL; ++m)
+#pragma unroll
+                    for (int q = 0; q < RL; ++q) {
+                        const int k = last_index<N>(i, m, q);
+                        if (k < nkx && 2 * k <= N) {
+                            const cplx zk = v[last_reg<N>(m, q)];
+                            const cplx zm = (k == 0) ? zk : buf[k];
+                            A[k] = make_double2(s * (zk.x + zm.x), s * (zk.y - zm.y));
+                            B[k] = make_double2(s * (zk.y + zm.y), s * (zm.x - zk.x));
+                        }
+                    }
+            }
+            team_sync<TP>(team);
+        }
+    }
+}
+
 template <int N> static cudaError_t launch_xrows_n(bool inverse, const RowArgs& a, const cplx* tw, cudaStream_t st) {
+    static DeviceOnce once;
+    const int dev = device_slot();
+    if (dev < 0) return cudaErrorInvalidDevice;
+    int sms = 0;
+    cudaError_t e = device_sm_count(dev, &sms);
+    if (e != cudaSuccess) return e;
     if constexpr (Plan<N>::E != 8) {
-        return cudaErrorInvalidValue;
+        using RC = XRowGenCfg<N>;
+        if (!once.done[dev]) {
+            e = cudaFuncSetAttribute(xrows_general_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(xrows_general_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
+            if (e != cudaSuccess) return e;
+            once.done[dev] = true;
+        }
+        const long long groups = ((a.nrows + 1) / 2 + RC::TEAMS - 1) / RC::TEAMS;
+        const long long cap = (long long)sms * 8;
+        const unsigned blocks = (unsigned)(groups < cap ? groups : cap);
+        if (inverse) xrows_general_kernel<N, true><<<blocks, RC::THREADS, RC::SMEM, st>>>(a, tw);
+        else xrows_general_kernel<N, false><<<blocks, RC::THREADS, RC::SMEM, st>>>(a, tw);
+        count_launch();
+        return cudaGetLastError();
     } else {
         using RC = XRowCfg<N>;
-        static int sms = 0;
-        if (sms == 0) {
-            int dev = 0;
-            cudaError_t e = cudaGetDevice(&dev);
-            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(xrows_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
+        if (!once.done[dev]) {
+            e = cudaFuncSetAttribute(xrows_kernel<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(xrows_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
-            if (e != cudaSuccess) { sms = 0; return e; }
+            if (e != cudaSuccess) return e;
+            once.done[dev] = true;
         }
         const long long groups = ((a.nrows + 1) / 2 + RC::TEAMS - 1) / RC::TEAMS;
         const long long cap = (long long)sms * 8;             // persistent; more CTAs than can be resident simply queue
@@ -546,14 +569,9 @@ template <int N> static cudaError_t launch_xrows_n(bool inverse, const RowArgs& 
 
 cudaError_t launch_xrows(int n, bool inverse, const RowArgs& a, const double2* tw, cudaStream_t st) {
     switch (n) {
-        case 8: return launch_xrows_n<8>(inverse, a, tw, st);
-        case 16: return launch_xrows_n<16>(inverse, a, tw, st);
-        case 32: return launch_xrows_n<32>(inverse, a, tw, st);
-        case 64: return launch_xrows_n<64>(inverse, a, tw, st);
-        case 128: return launch_xrows_n<128>(inverse, a, tw, st);
-        case 256: return launch_xrows_n<256>(inverse, a, tw, st);
-        case 512: return launch_xrows_n<512>(inverse, a, tw, st);
-        case 1024: return launch_xrows_n<1024>(inverse, a, tw, st);
+#define X(N_) case N_: return launch_xrows_n<N_>(inverse, a, tw, st);
+        X(8) X(12) X(16) X(24) X(32) X(48) X(64) X(96) X(128) X(192) X(256) X(384) X(512) X(768) X(1024)
+#undef X
         default: return cudaErrorInvalidValue;
     }
 }
@@ -568,16 +586,19 @@ template <int N> static cudaError_t launch_xfused_n(const XFusedArgs& a, int hyd
         const bool pruned = a.nkx <= 3 * CF::TP;
         const size_t smem = CF::SMEM + (pruned ? sizeof(cplx) * (size_t)CF::TEAMS * 4 * a.px + 16 * (size_t)CF::TEAMS : 0);
         if (smem > kMaxSmem) return cudaErrorInvalidValue;
-        static int sms = 0;
-        if (sms == 0) {
-            int dev = 0;
-            cudaError_t e = cudaGetDevice(&dev);
-            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(xfused_kernel<N, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
+        static DeviceOnce once;
+        const int dev = device_slot();
+        if (dev < 0) return cudaErrorInvalidDevice;
+        int sms = 0;
+        cudaError_t e = device_sm_count(dev, &sms);
+        if (e != cudaSuccess) return e;
+        if (!once.done[dev]) {
+            e = cudaFuncSetAttribute(xfused_kernel<N, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(xfused_kernel<N, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(xfused_kernel<N, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(xfused_kernel<N, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
-            if (e != cudaSuccess) { sms = 0; return e; }
+            if (e != cudaSuccess) return e;
+            once.done[dev] = true;
         }
         // persistent: one CTA per SM, or fewer when there are not enough rows; several CTAs per SM for the small lengths
         const long long groups = (a.nrows + CF::TEAMS - 1) / CF::TEAMS;

@@ -244,14 +244,16 @@ template <int N> static cudaError_t launch_zstage_n(const ZStageArgs& a, const c
     if constexpr (Plan<N>::E != 8 || N > 512) {
         return cudaErrorInvalidValue;
     } else {
-        static bool attr_done = false;
-        if (!attr_done) {
+        static DeviceOnce once;
+        const int dev = device_slot();
+        if (dev < 0) return cudaErrorInvalidDevice;
+        if (!once.done[dev]) {
             cudaError_t e = cudaFuncSetAttribute(zstage_kernel<N, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZTile<N>::SMEM);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(zstage_kernel<N, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZTile<N>::SMEM);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(zstage_kernel<N, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZTile<N>::SMEM);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(zstage_kernel<N, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZTile<N>::SMEM);
             if (e != cudaSuccess) return e;
-            attr_done = true;
+            once.done[dev] = true;
         }
         const unsigned blocks = (unsigned)((a.inner + ZTile<N>::COLS - 1) / ZTile<N>::COLS);
         if (a.st.mode == STAGE_AB2) {

@@ -226,3 +226,21 @@ def smooth_random_state(nx, ny, nz, seed, kmax=2.0, hydro=False):
     else:
         b = random_phase_solenoidal(nx, ny, nz, kmax, 0.3, rng)
     return [rho, u[0], u[1], u[2], b[0], b[1], b[2]]
+
+
+def full_band_state(nx, ny, nz, seed, hydro=False):
+    """White noise under a smooth envelope: O(1) content in EVERY Fourier mode up to the Nyquist index, so that the
+    modes next to the 2/3-rule cut (index 170/171 on a 512 axis) and every pruned-index path carry full-size data.
+    rho = 1 + 0.3 e(x) w(x) stays in [0.7, 1.3] on the grid (w uniform in [-1,1), e in [0.25, 1] a k = 1 cosine product);
+    u and B are e(x) times independent uniform noise of amplitude 1 and 0.5.  Test input only (not a paper workload)."""
+    rng = np.random.default_rng(seed)
+    x, y, z = grid(nx, ny, nz)
+    env = 0.25 + 0.75 * (0.5 + 0.5 * np.cos(x + 0.3)) * (0.5 + 0.5 * np.cos(y - 1.1)) * (0.5 + 0.5 * np.cos(z + 2.0))
+    shape = (nz, ny, nx)
+    rho = 1.0 + 0.3 * env * rng.uniform(-1.0, 1.0, size=shape)
+    u = [env * rng.uniform(-1.0, 1.0, size=shape) for _ in range(3)]
+    if hydro:
+        b = [np.zeros(shape) for _ in range(3)]
+    else:
+        b = [0.5 * env * rng.uniform(-1.0, 1.0, size=shape) for _ in range(3)]
+    return [np.ascontiguousarray(a) for a in [rho] + u + b]

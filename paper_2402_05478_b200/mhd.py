@@ -16,14 +16,16 @@ LIB_PATH = os.path.join(_HERE, "libmhd_b200.so")
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = 0, -1, -2, -3, -4, -5
 AB2, RK4 = 0, 1
 FLAG_HYDRO, FLAG_NO_DEALIAS, FLAG_FORCING = 1, 2, 4
+FLAG_UNFUSED_X, FLAG_NO_GRAPH, FLAG_FUSED_ZSTAGE = 8, 16, 32
 
 EXPORTS = [
     "mhd_workspace_bytes", "mhd_create", "mhd_destroy", "mhd_set_fields", "mhd_set_fields_host", "mhd_set_box",
     "mhd_set_forcing", "mhd_set_forcing_host", "mhd_step",
     "mhd_state_bytes", "mhd_get_state", "mhd_set_state",
     "mhd_get_fields", "mhd_get_fields_host", "mhd_diagnostics", "mhd_strerror", "mhd_last_error",
-    "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy",
+    "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy", "mhd_fft_last_error",
     "mhd_launch_count", "mhd_profile_kernel_count", "mhd_profile_kernel_name", "mhd_profile_begin", "mhd_profile_end",
+    "mhd_measure_peaks",
 ]
 
 
@@ -81,18 +83,36 @@ def lib():
         L.mhd_fft_c2r.argtypes = [_vp, _vp, _vp]
         L.mhd_fft_plan_destroy.argtypes = [_vp]
         L.mhd_fft_plan_destroy.restype = None
+        L.mhd_fft_last_error.restype = C.c_char_p
+        L.mhd_fft_last_error.argtypes = [_vp]
         L.mhd_launch_count.restype = C.c_longlong
         L.mhd_profile_kernel_count.restype = C.c_int
         L.mhd_profile_kernel_name.restype = C.c_char_p
         L.mhd_profile_kernel_name.argtypes = [C.c_int]
         L.mhd_profile_begin.argtypes = [_vp]
         L.mhd_profile_end.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
+        L.mhd_measure_peaks.argtypes = [_vp, C.c_size_t, _vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
 
 def launch_count() -> int:
     return int(lib().mhd_launch_count())
+
+
+def measure_peaks(device="cuda:0"):
+    """(FP64 TFLOP/s, shared-memory GB/s) measured on `device` by the library's own probe kernels (mhd_measure_peaks)."""
+    torch = _torch()
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        scratch = torch.empty(8 << 20, dtype=torch.uint8, device=dev)
+        f, s = C.c_double(), C.c_double()
+        torch.cuda.synchronize(dev)
+        rc = lib().mhd_measure_peaks(_vp(scratch.data_ptr()), scratch.numel(), _vp(torch.cuda.current_stream(dev).cuda_stream),
+                                     C.byref(f), C.byref(s))
+    if rc != OK:
+        raise MhdError(rc, "mhd_measure_peaks")
+    return float(f.value), float(s.value)
 
 
 def _torch():
@@ -196,9 +216,14 @@ class Solver:
         return rc
 
     def close(self):
+        """mhd_step is asynchronous on the solver's own stream: wait for it before the context is destroyed and the
+        workspace goes back to torch's caching allocator (which could hand it to another stream at once)."""
         if getattr(self, "_h", None):
-            lib().mhd_destroy(self._h)
-            self._h = _vp()
+            try:
+                self._stream.synchronize()
+            finally:
+                lib().mhd_destroy(self._h)
+                self._h = _vp()
         self._ws = None
 
     def __del__(self):
@@ -328,7 +353,7 @@ class FftPlan:
         rc = lib().mhd_fft_r2c(self._h, _dev_ptr(real, n, "real"), _vp(out.data_ptr()))
         torch.cuda.current_stream(self.device).wait_stream(self._stream)
         if rc != OK:
-            raise MhdError(rc, "mhd_fft_r2c")
+            raise MhdError(rc, "mhd_fft_r2c", lib().mhd_fft_last_error(self._h).decode())
         return out
 
     def c2r(self, spec, out=None):
@@ -341,13 +366,16 @@ class FftPlan:
         rc = lib().mhd_fft_c2r(self._h, _vp(spec.data_ptr()), _vp(out.data_ptr()))
         torch.cuda.current_stream(self.device).wait_stream(self._stream)
         if rc != OK:
-            raise MhdError(rc, "mhd_fft_c2r")
+            raise MhdError(rc, "mhd_fft_c2r", lib().mhd_fft_last_error(self._h).decode())
         return out
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().mhd_fft_plan_destroy(self._h)
-            self._h = _vp()
+            try:
+                self._stream.synchronize()      # transforms may still be running on the plan's stream
+            finally:
+                lib().mhd_fft_plan_destroy(self._h)
+                self._h = _vp()
         self._ws = None
 
     def __del__(self):

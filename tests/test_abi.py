@@ -93,3 +93,27 @@ def test_product_package_never_imports_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle", text, flags=re.M), f
                 assert "mhd_ref" not in text and "oracle/" not in text and "oracle." not in text, f
+
+
+def test_library_has_no_hidden_dispatch_and_no_per_process_device_state():
+    """The ABI is the only way to choose an execution plan (mhd_create flags): no translation unit reads the environment,
+    and kernel attributes / SM counts are cached per DEVICE (DeviceOnce keyed by cudaGetDevice), never in a per-process
+    static, so two contexts on two GPUs of one process cannot share a launch configuration by accident."""
+    csrc = os.path.join(ROOT, "paper_2402_05478_b200", "csrc")
+    for f in os.listdir(csrc):
+        text = open(os.path.join(csrc, f)).read()
+        assert "getenv" not in text, f
+        assert not re.search(r"static\s+(int\s+sms|bool\s+attr_done)", text), f
+    internal = open(os.path.join(csrc, "mhd_internal.h")).read()
+    assert "struct DeviceOnce" in internal and "kMaxDevices" in internal
+    for f in ("fft_kernels.cu", "xfused_kernel.cu", "zstage_kernel.cu"):
+        text = open(os.path.join(csrc, f)).read()
+        assert text.count("cudaFuncSetAttribute") > 0 and "once.done[dev]" in text, f
+
+
+def test_peaks_probe_rejects_bad_arguments(lib):
+    from paper_2402_05478_b200 import mhd
+    f, s = C.c_double(), C.c_double()
+    assert lib.mhd_measure_peaks(None, 1 << 23, None, C.byref(f), C.byref(s)) == mhd.EINVAL
+    assert lib.mhd_measure_peaks(C.c_void_p(256), 16, None, C.byref(f), C.byref(s)) == mhd.EINVAL
+    assert lib.mhd_fft_last_error(None) == b""

@@ -154,15 +154,14 @@ def test_paper_diagnostics_on_config1_and_closed_forms(gpu, ref):
 
 
 @pytest.mark.parametrize("integrator,hydro", [(0, False), (1, False), (0, True)])
-def test_fused_z_forward_stage_kernel_matches_oracle(gpu, ref, integrator, hydro, monkeypatch):
-    """the opt-in fused z-forward + stage kernel (zstage_kernel.cu, MHD_ZFUSE=1): same results as the oracle,
+def test_fused_z_forward_stage_kernel_matches_oracle(gpu, ref, integrator, hydro):
+    """the fused z-forward + stage kernel (zstage_kernel.cu, MHD_FLAG_FUSED_ZSTAGE): same results as the oracle,
     with forcing and a stretched box, Euler start + steady AB2 (graph replay) or RK4."""
     import torch
-    monkeypatch.setenv("MHD_ZFUSE", "1")
     shape = (32, 16, 64)
     f = inputs.smooth_random_state(64, 16, 32, seed=41, hydro=hydro)
     force = [0.05 * np.cos(np.arange(64) * TWO_PI / 64)[None, None, :] * np.ones(shape), np.zeros(shape), 0.02 * np.ones(shape)]
-    flags = gpu.FLAG_FORCING | (gpu.FLAG_HYDRO if hydro else 0)
+    flags = gpu.FLAG_FORCING | gpu.FLAG_FUSED_ZSTAGE | (gpu.FLAG_HYDRO if hydro else 0)
     o, g = both(gpu, ref, shape, f, 3e-3, 2e-3, 1.1, 1e-3, integrator=integrator, flags=flags, box=(TWO_PI, 3.0, 5.0), force=force)
     launches0 = gpu.launch_count()
     o.step(1); g.step(1)
@@ -176,6 +175,55 @@ def test_fused_z_forward_stage_kernel_matches_oracle(gpu, ref, integrator, hydro
     if not hydro:
         assert rel(got[4:7], want[4:7]) <= 1e-12
     assert gpu.launch_count() > launches0
+
+
+def test_execution_plan_flags_do_not_change_the_result(gpu, ref):
+    """MHD_FLAG_NO_GRAPH is bit-identical to the default plan (same kernels, launched one by one); MHD_FLAG_UNFUSED_X (x C2R,
+    products kernel, x R2C through real arrays) and MHD_FLAG_FUSED_ZSTAGE agree with it to roundoff and with the oracle at
+    the per-step bar.  Nothing is selected through the environment."""
+    import torch
+    cfg = inputs.config1()
+    dev = [torch.from_numpy(a).cuda() for a in cfg.arrays()]
+    res = {}
+    for name, fl in (("default", 0), ("nograph", gpu.FLAG_NO_GRAPH), ("unfused", gpu.FLAG_UNFUSED_X), ("zstage", gpu.FLAG_FUSED_ZSTAGE),
+                     ("all", gpu.FLAG_NO_GRAPH | gpu.FLAG_UNFUSED_X | gpu.FLAG_FUSED_ZSTAGE)):
+        s = gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, flags=fl)
+        s.set_fields(*dev); s.step(9)
+        res[name] = [t.cpu().numpy() for t in s.get_fields()]
+    for a, b in zip(res["default"], res["nograph"]):
+        assert np.array_equal(a, b)
+    o = ref.RefSolver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
+    o.set_fields(*cfg.arrays()); o.step(9)
+    want = o.get_fields()
+    for name in ("unfused", "zstage", "all"):
+        assert rel(res[name], res["default"]) <= 1e-13, name
+        assert rel(res[name], want) <= 1e-12, name
+    with pytest.raises(gpu.MhdError):
+        gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, flags=1 << 20)      # unknown flag bits are refused
+
+
+def test_solver_runs_while_the_current_stream_and_device_context_differ(gpu):
+    """every ABI call makes the workspace's device current for its own duration (DeviceGuard) and enqueues on the context's
+    stream only: driving a solver from inside another stream context, and closing it right after an asynchronous step,
+    must neither fail nor corrupt a tensor allocated immediately afterwards (close() synchronises the private stream)."""
+    import torch
+    cfg = inputs.config1()
+    dev = [torch.from_numpy(a).cuda() for a in cfg.arrays()]
+    a = gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
+    a.set_fields(*dev); a.step(40)
+    want = [t.clone() for t in a.get_fields()]
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        b = gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
+        b.set_fields(*dev); b.step(40)
+        got = b.get_fields()
+        b.step(200)                   # asynchronous work still in flight ...
+        b.close()                     # ... when the context and its workspace are released
+        junk = torch.full((b.workspace_bytes // 8,), 7.0, dtype=torch.float64, device="cuda")   # likely reuses the block
+    torch.cuda.synchronize()
+    for x, y in zip(want, got):
+        assert torch.equal(x, y)
+    assert bool((junk == 7.0).all())
 
 
 @pytest.mark.parametrize("integrator", [0, 1])

@@ -55,6 +55,16 @@ def test_batched_3d_and_2d(gpu, ref, shape, batch):
     check(gpu, ref, shape, batch)
 
 
+@pytest.mark.parametrize("shape,batch", [((8, 512, 512), 3), ((12, 256, 256), 3), ((24, 64, 64), 1), ((8, 128, 128), 1),
+                                         ((1, 512, 512), 1), ((48, 128, 128), 5)])
+def test_plane_pipelined_xy_pass_against_the_oracle(gpu, ref, shape, batch):
+    """square (x,y) planes of 64..512 take the persistent plane-pipelined kernel (x and y passes meet in an L2-resident ring,
+    planefft_kernel.cu): plane counts that do not fill the last group, a single plane, more groups than ring slots; twice in
+    a row on the same plan (the ring and the counters are reused)."""
+    check(gpu, ref, shape, batch)
+    check(gpu, ref, shape, batch)
+
+
 @pytest.mark.parametrize("n", [256, 512, 768])
 def test_round_trip_at_bench_sizes(gpu, n):
     """config 5 sizes the oracle cannot finish in seconds: round trip and Parseval hold at any size."""

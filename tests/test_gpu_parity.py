@@ -67,9 +67,17 @@ def check_diag(dg, do, nshell=0):
     assert np.max(np.abs(dg["bmean"] - do["bmean"])) <= 1e-13
     assert abs(dg["max_divb"] - do["max_divb"]) <= 1e-12
     if nshell:
+        # per shell, RELATIVE: a shell value is a sum of |v^(k)|^2 whose amplitudes carry the transform's absolute
+        # roundoff delta ~ 1e-15 * sqrt(peak shell) (an FFT's error scales with the norm of the whole field, not of the
+        # mode), so |d E_s| <= 1e-10 E_s + 2 sqrt(E_s) delta n_s^(1/2) + delta^2 n_s; shells far below the peak are therefore
+        # still held to 1e-10 of THEIR OWN value until they sink under ~1e-20 of the peak.
         for k in ("ekin_spec", "emag_spec"):
-            scale = max(np.max(np.abs(do[k])), 1e-300)
-            assert np.max(np.abs(dg[k] - do[k])) <= ENERGY * scale, k
+            want, got = np.asarray(do[k]), np.asarray(dg[k])
+            peak = max(float(np.max(np.abs(want))), 1e-300)
+            delta2 = 1e-28 * peak
+            tol = ENERGY * np.abs(want) + 2.0 * np.sqrt(np.abs(want) * delta2) + delta2
+            bad = np.abs(got - want) > tol
+            assert not bad.any(), (k, np.nonzero(bad)[0][:5], got[bad][:5], want[bad][:5])
 
 
 # ------------------------------------------------------------------------------------------------
@@ -251,28 +259,67 @@ def test_config4_512_properties_and_sampled_parity(gpu, ref):
 
 @pytest.mark.slow
 def test_config4_512_sampled_parity_against_the_oracle_on_the_shared_grid(gpu, ref):
-    """Full-size parity in the launch configuration bench.py times, on sampled outputs the oracle can compute.
+    """Full-size parity in the launch configuration bench.py times, on sampled outputs the oracle can compute, over the
+    config's FULL step count (north_star: <= 1e-11 per step, <= 1e-8 after the config's 100 steps, energies 1e-10).
     Config 4's initial state is band-limited to |k| <= 32, so the same physical state lives exactly on a 256^3 grid
-    (every second point).  One Euler step only creates modes |k| <= 64, inside both masks (85 at 256, 170 at 512),
-    and later steps put < 1e-30 beyond mode 85: the 512^3 GPU fields at the even grid points must equal the
-    256^3 oracle fields to roundoff, and the volume-averaged energies (band-limited integrands) must agree too."""
+    (every second point).  As long as the solution keeps negligible content beyond index 85 (the 256^3 mask; the 512^3
+    mask is 170) the two discretisations solve the same ODE system mode by mode: the 512^3 GPU fields at the even grid
+    points must equal the 256^3 oracle fields to roundoff.  That premise is checked ON THE ORACLE ALONE (its shell
+    spectra next to its own cut, printed) before the comparison is trusted."""
     n = int(os.environ.get("MHD_BIG_N", "512"))
+    steps = int(os.environ.get("MHD_BIG_STEPS", "100"))
     h = n // 2
-    cfg = inputs.config4(n, 100)
+    cfg = inputs.config4(n, steps)
     g = gpu.Solver(n, n, n, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
     g.set_fields_host(*cfg.arrays())
     o = ref.RefSolver(h, h, h, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
     o.set_fields(*[np.ascontiguousarray(a[::2, ::2, ::2]) for a in cfg.arrays()])
     g.step(1); o.step(1)
     got = [np.ascontiguousarray(a[::2, ::2, ::2]) for a in g.get_fields_host()]
-    assert max(group_errors(got, o.get_fields())) <= PER_STEP
-    g.step(5); o.step(5)            # steps 4.. are CUDA-graph replays, exactly what bench.py times
+    e1 = max(group_errors(got, o.get_fields()))
+    assert e1 <= PER_STEP, e1
+    g.step(steps - 1); o.step(steps - 1)      # steps 4.. are CUDA-graph replays, exactly what bench.py times
+    # premise, on the oracle alone: content next to the 256^3 cut (|k| = 85) relative to the spectral peak
+    kcut = (h - 1) // 3
+    do = o.diagnostics(kcut + 1)
+    tail = max(float(np.max(do["ekin_spec"][kcut - 5:])), float(np.max(do["emag_spec"][kcut - 5:])))
+    peak = max(float(np.max(do["ekin_spec"])), float(np.max(do["emag_spec"])))
+    print(f"config4 shared grid: oracle {h}^3 after {steps} steps, shells {kcut - 5}..{kcut}: {tail:.3e} of peak {peak:.3e}"
+          f" (ratio {tail / peak:.1e}); one-step error {e1:.2e}")
+    assert tail <= 1e-26 * peak, "the solution has reached the 256^3 cut: the shared-grid comparison no longer applies"
     got = [np.ascontiguousarray(a[::2, ::2, ::2]) for a in g.get_fields_host()]
-    assert max(group_errors(got, o.get_fields())) <= 1e-10
-    dg, do = g.diagnostics(0), o.diagnostics(0)
+    err = max(group_errors(got, o.get_fields()))
+    print(f"config4 shared grid: relative L2 error after {steps} steps {err:.2e}")
+    assert err <= END_OF_RUN, err
+    dg = g.diagnostics(0)
     for k in ("ekin", "emag", "mass"):
         assert abs(dg[k] - do[k]) <= ENERGY * abs(do[k]), (k, dg[k], do[k])
     assert abs(dg["enstrophy"] - do["enstrophy"]) <= 1e-9 * do["enstrophy"]
+    assert dg["step"] == steps
+
+
+@pytest.mark.parametrize("integrator", [0, 1])
+@pytest.mark.parametrize("shape", [(8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024), (8, 8, 768), (8, 768, 8)])
+def test_full_band_state_through_every_pruned_index_path(gpu, ref, shape, integrator):
+    """Production-length axes with O(1) energy in EVERY mode (white noise under a smooth envelope, rho in [0.7, 1.3]):
+    the modes next to the 2/3 cut (index 170 kept / 171 dropped at 512), the zero-filled band of the
+    inverse passes, the partially filled legs of the fused x pass and the Hermitian-split window all carry full-size
+    data, so an index slip anywhere in them is an O(1) error.  set -> get (mask only), then one step and a second step
+    (Euler start + AB2, or two RK4 steps) against the oracle at the per-step bar."""
+    import torch
+    nz, ny, nx = shape
+    f = inputs.full_band_state(nx, ny, nz, seed=31)
+    cfg = inputs.Config("fullband", nx, ny, nz, nu=0.01, eta=0.02, cs=1.0, dt=2e-4, steps=2)
+    cfg.fields = dict(zip(("rho", "ux", "uy", "uz", "bx", "by", "bz"), f))
+    o, g, e0 = run_both(gpu, ref, cfg, 0, integrator=integrator)
+    assert e0 <= 1e-13, e0
+    check_diag(g.diagnostics(64), o.diagnostics(64), 64)
+    for _ in range(2):
+        o.step(1); g.step(1)
+        got = [t.cpu().numpy() for t in g.get_fields()]
+        e = max(group_errors(got, o.get_fields()))
+        assert e <= PER_STEP, e
+    check_diag(g.diagnostics(64), o.diagnostics(64), 64)
 
 
 @pytest.mark.parametrize("shape", [(8, 8, 512), (8, 8, 1024), (8, 8, 256), (8, 8, 128), (8, 512, 8), (512, 8, 8), (16, 1024, 8)])

@@ -73,7 +73,10 @@ def test_abc_flow_energy_exchange_period(gpu):
 def test_orszag_tang_2d_energy_exchange_period(gpu):
     """Reading: A = 1, k0 = 1, u0 = 1, M_A = 1 (uniform B0 = 1 along x), Ms = 0.01 (Cs = 100), Re = Rm = 1000, 128^2,
     dt = 1e-4 (the paper's).  AB2 is unstable for sound waves at Cs kmax dt = 0.42 with no damping there, so RK4 is used.
-    The paper prints T = 2.971; pi/(k0 V_A) = 3.14; this code gives 3.14-3.18."""
+    The paper prints T = 2.971; pi/(k0 V_A) = 3.14; this code gives 3.14-3.18.  No reading of the unstated parameters
+    reproduces the printed value (measured on the GPU, round 2: B0 along y 3.18/3.13, B0 at 45 degrees 3.95, Re = Rm = 1e5
+    3.18/3.15, Re = 100 3.14/3.00, Ms = 0.1 3.24/3.14), so the assertion is the linear Alfven value pi/(k0 V_A) +- 3 %; the
+    printed period is only reported (it sits 5.4 % below that value; the paper's ABC period sits 4 % below its own)."""
     n = 128
     x = TWO_PI * np.arange(n) / n
     Y, X = np.meshgrid(x, x, indexing="ij")
@@ -83,8 +86,9 @@ def test_orszag_tang_2d_energy_exchange_period(gpu):
     pk = maxima(t, em)
     assert len(pk) >= 2
     T = pk[1] - pk[0]
-    assert abs(T - GOLD["period_2d_orszag_tang"]["value"]) <= 0.08 * GOLD["period_2d_orszag_tang"]["value"], T
-    assert abs(T - np.pi) <= 0.03 * np.pi
+    printed = GOLD["period_2d_orszag_tang"]["value"]
+    print(f"2-D OT exchange period {T:.4f}; pi/(k0 V_A) = {np.pi:.4f}; printed {printed} ({100 * (T - printed) / printed:+.1f} %)")
+    assert abs(T - np.pi) <= 0.03 * np.pi, T
     assert d["max_divb"] <= 1e-10
 
 
@@ -111,3 +115,63 @@ def test_config2_kelvin_helmholtz_growth_rate_on_the_gpu(gpu):
     want = kh_eig(256, 0.05, 4, c.nu, c.cs)[0].real
     assert abs(gam[4] - want) <= 0.05 * want, (gam, want)
     assert gam[4] > gam[2] > 0.0          # growth increases with kx below the maximum at kx a = 0.4
+
+
+def taylor_green(n):
+    """eq. (8), PAPER.md:190-196 (third line is u_z)"""
+    x = TWO_PI * np.arange(n) / n
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    return [np.ones((n, n, n)), np.cos(X) * np.sin(Y) * np.cos(Z), -np.sin(X) * np.cos(Y) * np.cos(Z), np.zeros((n, n, n))]
+
+
+def omega_series(gpu, n, re, tend, cs=10.0, dt=2e-3, every=50):
+    import torch
+    s = gpu.Solver(n, n, n, 1.0 / re, 0.0, cs, dt, integrator=gpu.RK4, flags=gpu.FLAG_HYDRO)
+    s.set_fields(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in taylor_green(n)])
+    d = s.diagnostics()
+    t, om = [0.0], [d["enstrophy"]]
+    for _ in range(int(round(tend / (dt * every)))):
+        s.step(every)
+        d = s.diagnostics()
+        assert d["rc"] == 0
+        t.append(d["time"]); om.append(d["enstrophy"])
+    return np.array(t), np.array(om)
+
+
+def test_taylor_green_mean_square_vorticity(gpu, ref):
+    """SURVEY.md §8(f) #3, the paper's Test 2 (eq. 8, Fig. 7): growth of the normalised
+    mean-square vorticity Omega(t)/Omega(0) of the 3-D Taylor-Green vortex at Re = 300 and 400.  Reading: hydro flag,
+    u0 = 1, Ms = 0.1 (Cs = 10: "incompressible" limit), RK4, dt = 2e-3 (Cs kmax dt = 0.42).
+    (i) parity: the same run at 32^3 for 100 steps against the oracle, Omega(t) to 1e-10;
+    (ii) the paper's statements as weak pins on the 64^3 GPU run: Omega(0) = 3/4 exactly; a single maximum at Re = 300;
+    at Re = 400 a SECOND peak "at around t = 9" (found at t = 8.5 here); "64^3 suffices":
+    the 128^3 curve agrees with the 64^3 one to 3 % up to t = 9 (measured 1.8 %)."""
+    import torch
+    # (i) parity with the oracle
+    n = 32
+    f = taylor_green(n)
+    g = gpu.Solver(n, n, n, 1.0 / 400, 0.0, 10.0, 2e-3, integrator=gpu.RK4, flags=gpu.FLAG_HYDRO)
+    o = ref.RefSolver(n, n, n, 1.0 / 400, 0.0, 10.0, 2e-3, integrator=1, flags=1)
+    g.set_fields(*[torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in f])
+    o.set_fields(*(f + [np.zeros((n, n, n))] * 3))
+    for _ in range(4):
+        g.step(25); o.step(25)
+        dg, do = g.diagnostics(), o.diagnostics()
+        assert abs(dg["enstrophy"] - do["enstrophy"]) <= 1e-10 * do["enstrophy"]
+        assert abs(dg["ekin"] - do["ekin"]) <= 1e-10 * do["ekin"]
+    # (ii) the paper's curves
+    t3, om3 = omega_series(gpu, 64, 300, 12.0)
+    t4, om4 = omega_series(gpu, 64, 400, 12.0)
+    assert abs(om3[0] - 0.75) <= 1e-12 and abs(om4[0] - 0.75) <= 1e-12        # <|curl u|^2> of eq. (8) is 3/4
+    r3, r4 = om3 / om3[0], om4 / om4[0]
+    pk3 = [p for p in maxima(t3, r3) if 2.0 < p < 11.5]
+    pk4 = [p for p in maxima(t4, r4) if 2.0 < p < 11.5]
+    print(f"TG 64^3: Re=300 max {r3.max():.3f} at t={t3[r3.argmax()]:.1f}, peaks {np.round(pk3, 2)}; "
+          f"Re=400 max {r4.max():.3f} at t={t4[r4.argmax()]:.1f}, peaks {np.round(pk4, 2)}")
+    assert len(pk3) == 1 and 5.5 <= pk3[0] <= 7.0, pk3
+    assert len(pk4) == 2 and 6.0 <= pk4[0] <= 7.8 and 8.0 <= pk4[1] <= 9.5, pk4     # "secondary peak ... at around t = 9"
+    assert r4.max() > r3.max() > 4.0                                             # growth increases with Re
+    tb, omb = omega_series(gpu, 128, 400, 9.0, every=50)
+    rb = omb / omb[0]
+    m = len(tb)
+    assert np.max(np.abs(rb - r4[:m]) / rb) <= 0.03                              # 64^3 already reproduces the curve
