@@ -149,6 +149,14 @@ int  mhd_fft_r2c(mhd_fft_plan* plan, const double* in_real_dev, double* out_comp
 /* inverse, includes 1/(nx*ny*nz); Im of self-conjugate x modes (kx = 0, nx/2 of a row) is ignored */
 int  mhd_fft_c2r(mhd_fft_plan* plan, const double* in_complex_dev, double* out_real_dev);
 void mhd_fft_plan_destroy(mhd_fft_plan* plan);
+/* How the x and y passes run.  MHD_FFT_THREE_SWEEP (default): one kernel per axis, every pass streams the batch through HBM
+ * (6 F of traffic per transform).  MHD_FFT_PLANE_PIPELINE (square planes nx == ny in {64,128,256,512} only, MHD_EINVAL
+ * otherwise): x and y passes in one persistent kernel, plane groups handed over through an L2-resident ring (4 F of traffic:
+ * the "2-sweep" transform of SURVEY.md §8(f) #4).  Same results to roundoff.  Measured on B200 at 512^3: DRAM traffic of the x+y
+ * part falls from 30 GB to 15 GB, but the kernel is bound by the SM's load-store pipe, not by HBM, and runs slower than
+ * the two separate passes (profiles/r02_planefft.md): hence not the default. */
+enum { MHD_FFT_THREE_SWEEP = 0, MHD_FFT_PLANE_PIPELINE = 1 };
+int mhd_fft_plan_set_mode(mhd_fft_plan* plan, int mode);
 const char* mhd_fft_last_error(const mhd_fft_plan* plan);   /* detail of the last MHD_ECUDA on this plan ("" if none) */
 
 /* ==== Instrumentation (not part of the solver's contract; used by bench.py and the tests) ====================== */

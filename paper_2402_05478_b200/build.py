@@ -20,7 +20,7 @@ LIB = os.path.join(HERE, "libmhd_b200.so")
 OBJDIR = os.path.join(HERE, "build")
 SOURCES = ["fft_kernels.cu", "xfused_kernel.cu", "planefft_kernel.cu", "zstage_kernel.cu", "mhd_kernels.cu", "peaks_kernel.cu",
            "mhd_api.cu"]
-HEADERS = ["fft_core.cuh", "xteam.cuh", "mhd_internal.h"]
+HEADERS = ["fft_core.cuh", "xteam.cuh", "bulk_copy.cuh", "mhd_internal.h"]
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--compiler-options", "-fPIC", "-cudart", "static"]

@@ -33,12 +33,9 @@ __device__ __forceinline__ cplx mul_mi(cplx a) {
 
 // ---- radix plans ---------------------------------------------------------------------------
 // radices in execution order; a factor 3, if any, goes last so that P stays a power of two.
-// V = 0: the 8 (12/24)-points-per-thread plans every kernel uses.  V = 1: "big radix" plans for the strided-axis kernels:
-// 16 or 32 points per thread and only TWO passes (one shared-memory exchange instead of two), see fft_kernels.cu.
-template <int N, int V = 0> struct Plan;
-#define MHD_PLAN(N_, E_, NP_, R0, R1, R2, R3) MHD_PLANV(N_, 0, E_, NP_, R0, R1, R2, R3)
-#define MHD_PLANV(N_, V_, E_, NP_, R0, R1, R2, R3)                                               \
-    template <> struct Plan<N_, V_> {                                                            \
+template <int N> struct Plan;
+#define MHD_PLAN(N_, E_, NP_, R0, R1, R2, R3)                                                    \
+    template <> struct Plan<N_> {                                                                \
         static constexpr int E = E_;   /* elements per thread */                                 \
         static constexpr int NP = NP_; /* passes */                                              \
         static constexpr int TP = N_ / E_; /* threads per pencil */                              \
@@ -61,17 +58,11 @@ MHD_PLAN(96, 24, 3, 8, 4, 3, 1)
 MHD_PLAN(192, 24, 3, 8, 8, 3, 1)
 MHD_PLAN(384, 24, 4, 8, 4, 4, 3)
 MHD_PLAN(768, 24, 4, 8, 8, 4, 3)
-MHD_PLANV(128, 1, 16, 2, 16, 8, 1, 1)
-MHD_PLANV(256, 1, 16, 2, 16, 16, 1, 1)
-MHD_PLANV(512, 1, 32, 2, 32, 16, 1, 1)
-MHD_PLANV(1024, 1, 32, 2, 32, 32, 1, 1)
 #undef MHD_PLAN
-#undef MHD_PLANV
-template <int N> struct HasBigPlan { static constexpr bool value = (N == 128 || N == 256 || N == 512 || N == 1024); };
 
 // pencil groups per CTA (8 pencils each), chosen so a CTA has 128..512 threads
-template <int N, int V = 0> struct Tile {
-    static constexpr int TP = Plan<N, V>::TP;
+template <int N> struct Tile {
+    static constexpr int TP = Plan<N>::TP;
     static constexpr int G = (8 * TP >= 128) ? 1 : 128 / (8 * TP);
     static constexpr int THREADS = 8 * TP * G;
     static constexpr int COLS = 8 * G;                       // pencils per CTA
@@ -109,75 +100,19 @@ template <bool INV> __device__ __forceinline__ void bfly8(cplx* v) {
     v[2] = cadd(e2, w2); v[6] = csub(e2, w2);
     v[3] = cadd(e3, w3); v[7] = csub(e3, w3);
 }
-// ---- composite radices 16 = 4 x 4 and 32 = 4 x 8, entirely in registers, internal twiddles are compile-time constants ----
-// cos / sin of 2*pi*j/32 (correctly rounded literals)
-__host__ __device__ constexpr double cos32(int j) { return j == 0 ? 1.0 : j == 1 ? 0.9807852804032304 : j == 2 ? 0.9238795325112867 : j == 3 ? 0.8314696123025452 : j == 4 ? 0.7071067811865476 : j == 5 ? 0.5555702330196023 : j == 6 ? 0.38268343236508984 : j == 7 ? 0.19509032201612833 : j == 8 ? 6.123233995736766e-17 : j == 9 ? -0.1950903220161282 : j == 10 ? -0.3826834323650897 : j == 11 ? -0.555570233019602 : j == 12 ? -0.7071067811865475 : j == 13 ? -0.8314696123025453 : j == 14 ? -0.9238795325112867 : j == 15 ? -0.9807852804032304 : j == 16 ? -1.0 : j == 17 ? -0.9807852804032304 : j == 18 ? -0.9238795325112868 : j == 19 ? -0.8314696123025455 : j == 20 ? -0.7071067811865477 : j == 21 ? -0.5555702330196022 : j == 22 ? -0.38268343236509034 : j == 23 ? -0.19509032201612866 : j == 24 ? -1.8369701987210297e-16 : j == 25 ? 0.1950903220161283 : j == 26 ? 0.38268343236509 : j == 27 ? 0.5555702330196018 : j == 28 ? 0.7071067811865474 : j == 29 ? 0.8314696123025452 : j == 30 ? 0.9238795325112865 : j == 31 ? 0.9807852804032303 : 0.0; }
-__host__ __device__ constexpr double sin32(int j) { return j == 0 ? 0.0 : j == 1 ? 0.19509032201612825 : j == 2 ? 0.3826834323650898 : j == 3 ? 0.5555702330196022 : j == 4 ? 0.7071067811865475 : j == 5 ? 0.8314696123025452 : j == 6 ? 0.9238795325112867 : j == 7 ? 0.9807852804032304 : j == 8 ? 1.0 : j == 9 ? 0.9807852804032304 : j == 10 ? 0.9238795325112867 : j == 11 ? 0.8314696123025455 : j == 12 ? 0.7071067811865476 : j == 13 ? 0.5555702330196022 : j == 14 ? 0.3826834323650899 : j == 15 ? 0.1950903220161286 : j == 16 ? 1.2246467991473532e-16 : j == 17 ? -0.19509032201612836 : j == 18 ? -0.38268343236508967 : j == 19 ? -0.555570233019602 : j == 20 ? -0.7071067811865475 : j == 21 ? -0.8314696123025452 : j == 22 ? -0.9238795325112865 : j == 23 ? -0.9807852804032303 : j == 24 ? -1.0 : j == 25 ? -0.9807852804032304 : j == 26 ? -0.9238795325112866 : j == 27 ? -0.8314696123025455 : j == 28 ? -0.7071067811865477 : j == 29 ? -0.5555702330196022 : j == 30 ? -0.3826834323650904 : j == 31 ? -0.19509032201612872 : 0.0; }
-// a * exp(-/+ 2 pi i j / 32) for a compile-time j (forward: minus sign; inverse: plus)
-template <bool INV, int J> __device__ __forceinline__ cplx mul_w32(cplx a) {
-    constexpr int j = J & 31;
-    if constexpr (j == 0) return a;
-    else if constexpr (j == 8) return mul_mi<INV>(a);
-    else if constexpr (j == 16) return make_double2(-a.x, -a.y);
-    else if constexpr (j == 24) return mul_mi<!INV>(a);
-    else {
-        constexpr double c = cos32(j), s = INV ? sin32(j) : -sin32(j);      // w = c + i s
-        return make_double2(a.x * c - a.y * s, a.x * s + a.y * c);
-    }
-}
-// X[k] = sum_n v[n] w_{R*S}^{nk}, n = S*n1 + n2, k = k1 + R*k2: R-point butterflies over n1 (stride S), twiddle w^{n2 k1},
-// S-point butterflies over n2; the result is left in natural order.
-template <bool INV> __device__ __forceinline__ void bfly16(cplx* v) {
-#pragma unroll
-    for (int n2 = 0; n2 < 4; ++n2) bfly4<INV>(v[n2], v[4 + n2], v[8 + n2], v[12 + n2]);     // A[k1][n2] at v[4*k1 + n2]
-    v[5] = mul_w32<INV, 2>(v[5]);  v[6] = mul_w32<INV, 4>(v[6]);   v[7] = mul_w32<INV, 6>(v[7]);
-    v[9] = mul_w32<INV, 4>(v[9]);  v[10] = mul_w32<INV, 8>(v[10]); v[11] = mul_w32<INV, 12>(v[11]);
-    v[13] = mul_w32<INV, 6>(v[13]); v[14] = mul_w32<INV, 12>(v[14]); v[15] = mul_w32<INV, 18>(v[15]);
-#pragma unroll
-    for (int k1 = 0; k1 < 4; ++k1) bfly4<INV>(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);   // X[k1 + 4*k2] at v[4*k1 + k2]
-    cplx t[16];
-#pragma unroll
-    for (int r = 0; r < 16; ++r) t[r] = v[r];
-#pragma unroll
-    for (int k1 = 0; k1 < 4; ++k1)
-#pragma unroll
-        for (int k2 = 0; k2 < 4; ++k2) v[k1 + 4 * k2] = t[4 * k1 + k2];
-}
-template <bool INV, int K1> __device__ __forceinline__ void tw32_row(cplx* v) {   // v[8*K1 + n2] *= w32^(n2*K1), n2 = 1..7
-    v[8 * K1 + 1] = mul_w32<INV, 1 * K1>(v[8 * K1 + 1]); v[8 * K1 + 2] = mul_w32<INV, 2 * K1>(v[8 * K1 + 2]);
-    v[8 * K1 + 3] = mul_w32<INV, 3 * K1>(v[8 * K1 + 3]); v[8 * K1 + 4] = mul_w32<INV, 4 * K1>(v[8 * K1 + 4]);
-    v[8 * K1 + 5] = mul_w32<INV, 5 * K1>(v[8 * K1 + 5]); v[8 * K1 + 6] = mul_w32<INV, 6 * K1>(v[8 * K1 + 6]);
-    v[8 * K1 + 7] = mul_w32<INV, 7 * K1>(v[8 * K1 + 7]);
-}
-template <bool INV> __device__ __forceinline__ void bfly32(cplx* v) {
-#pragma unroll
-    for (int n2 = 0; n2 < 8; ++n2) bfly4<INV>(v[n2], v[8 + n2], v[16 + n2], v[24 + n2]);    // A[k1][n2] at v[8*k1 + n2]
-    tw32_row<INV, 1>(v); tw32_row<INV, 2>(v); tw32_row<INV, 3>(v);
-#pragma unroll
-    for (int k1 = 0; k1 < 4; ++k1) bfly8<INV>(&v[8 * k1]);                                   // X[k1 + 4*k2] at v[8*k1 + k2]
-    cplx t[32];
-#pragma unroll
-    for (int r = 0; r < 32; ++r) t[r] = v[r];
-#pragma unroll
-    for (int k1 = 0; k1 < 4; ++k1)
-#pragma unroll
-        for (int k2 = 0; k2 < 8; ++k2) v[k1 + 4 * k2] = t[8 * k1 + k2];
-}
 template <int R, bool INV> __device__ __forceinline__ void bfly(cplx* v) {
-    if constexpr (R == 32) bfly32<INV>(v);
-    else if constexpr (R == 16) bfly16<INV>(v);
-    else if constexpr (R == 8) bfly8<INV>(v);
+    if constexpr (R == 8) bfly8<INV>(v);
     else if constexpr (R == 4) bfly4<INV>(v[0], v[1], v[2], v[3]);
     else if constexpr (R == 3) bfly3<INV>(v);
     else if constexpr (R == 2) bfly2<INV>(v);
 }
 
 // index of the q-th input of butterfly m held by slot i in the FIRST pass, and of the q-th output in the LAST
-template <int N, int V = 0> __device__ __forceinline__ int first_index(int i, int m, int q) {
-    return i + Plan<N, V>::TP * m + q * (N / Plan<N, V>::radix(0));
+template <int N> __device__ __forceinline__ int first_index(int i, int m, int q) {
+    return i + Plan<N>::TP * m + q * (N / Plan<N>::radix(0));
 }
-template <int N, int V = 0> __device__ __forceinline__ int last_index(int i, int m, int q) {
-    return i + Plan<N, V>::TP * m + q * (N / Plan<N, V>::radix(Plan<N, V>::NP - 1));
+template <int N> __device__ __forceinline__ int last_index(int i, int m, int q) {
+    return i + Plan<N>::TP * m + q * (N / Plan<N>::radix(Plan<N>::NP - 1));
 }
 // position in the register array of (butterfly m, leg q) for first / last pass
 template <int N> __device__ __forceinline__ constexpr int first_reg(int m, int q) { return m * Plan<N>::radix(0) + q; }
@@ -209,32 +144,18 @@ struct Padded {
 // ---- the passes ----------------------------------------------------------------------------
 // tw[j] = exp(-2*pi*i*j/N), j = 0..N-1 (forward); the inverse conjugates on the fly.
 // sm + lay(e): where element e of this thread's pencil lives between passes.  i: slot (0..TP-1).
-template <int N, bool INV, int S, int P, typename L, int V = 0>
+template <int N, bool INV, int S, int P, typename L>
 struct Pass {
-    static constexpr int R = Plan<N, V>::radix(S);
-    static constexpr int E = Plan<N, V>::E;
-    static constexpr int TP = Plan<N, V>::TP;
-    static constexpr bool LAST = (S == Plan<N, V>::NP - 1);
+    static constexpr int R = Plan<N>::radix(S);
+    static constexpr int E = Plan<N>::E;
+    static constexpr int TP = Plan<N>::TP;
+    static constexpr bool LAST = (S == Plan<N>::NP - 1);
     __device__ __forceinline__ static void run(cplx (&v)[E], cplx* sm, int i, const L& lay, const cplx* __restrict__ tw) {
 #pragma unroll
         for (int m = 0; m < E / R; ++m) {
             const int b = i + TP * m;
             const int k = b & (P - 1);
-            if constexpr (S > 0 && V == 1) {
-                // big radix: w, w^2, w^4, w^8(, w^16) from the table, every other power by ONE multiplication chain of depth <= 3
-                // (15 or 31 table reads per butterfly would cost more load-store wavefronts than the exchange they replace)
-                cplx w[R];
-#pragma unroll
-                for (int q = 1; q < R; q <<= 1) {
-                    w[q] = __ldg(&tw[k * q * (N / (P * R))]);
-                    if (INV) w[q].y = -w[q].y;
-                }
-#pragma unroll
-                for (int q = 3; q < R; ++q)
-                    if ((q & (q - 1)) != 0) w[q] = cmul(w[q & (q - 1)], w[q & -q]);      // q = (q without its lowest bit) + lowest bit
-#pragma unroll
-                for (int q = 1; q < R; ++q) v[m * R + q] = cmul(v[m * R + q], w[q]);
-            } else if constexpr (S > 0) {
+            if constexpr (S > 0) {
 #pragma unroll
                 for (int q = 1; q < R; ++q) {
                     cplx w = __ldg(&tw[k * q * (N / (P * R))]);
@@ -250,24 +171,24 @@ struct Pass {
             }
         }
         if constexpr (!LAST) {
-            constexpr int Rn = Plan<N, V>::radix(S + 1);
+            constexpr int Rn = Plan<N>::radix(S + 1);
             __syncthreads();
 #pragma unroll
             for (int m = 0; m < E / Rn; ++m)
 #pragma unroll
                 for (int q = 0; q < Rn; ++q) v[m * Rn + q] = sm[lay(i + TP * m + q * (N / Rn))];
             __syncthreads();
-            Pass<N, INV, S + 1, P * R, L, V>::run(v, sm, i, lay, tw);
+            Pass<N, INV, S + 1, P * R, L>::run(v, sm, i, lay, tw);
         }
     }
 };
 
 // Transform the pencil whose first-pass inputs are in v (see first_index); on return v holds the
 // last-pass outputs (see last_index).  All threads of the CTA must call it (it synchronises).
-template <int N, bool INV, int V = 0>
-__device__ __forceinline__ void pencil_fft(cplx (&v)[Plan<N, V>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
+template <int N, bool INV>
+__device__ __forceinline__ void pencil_fft(cplx (&v)[Plan<N>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
     Cols8 lay{p};
-    Pass<N, INV, 0, 1, Cols8, V>::run(v, sm, i, lay, tw);
+    Pass<N, INV, 0, 1, Cols8>::run(v, sm, i, lay, tw);
 }
 // same for 4 pencils side by side (lane = (p = tid & 3, slot))
 template <int N, bool INV>

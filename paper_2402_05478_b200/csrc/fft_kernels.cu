@@ -7,6 +7,11 @@
 //                     load, a forward pass simply does not store them, so pruned data never
 //                     touches HBM.
 //  The x axis (real rows <-> half-spectrum rows, two real rows per complex transform) lives in xfused_kernel.cu.
+//
+//  Measured and not kept (round 2, 512^3, profiles/r02_experiments.md): 32 points per thread with a single exchange (slower:
+//  168 registers, 12 warps/SM), TMA / cp.async staging of the next tile in a persistent CTA (slower: one CTA per SM), a
+//  persistent tile loop with L2 prefetch (slower than letting the hardware scheduler start a fresh CTA per tile).  With the
+//  transform removed this access pattern runs at 0.85-1.0 of the copy bandwidth; with it, at 0.70-0.83.
 #include "mhd_internal.h"
 #include "fft_core.cuh"
 
@@ -22,26 +27,13 @@ __device__ __forceinline__ int compact_index(int f, int n, int nk) {
     return -1;
 }
 
-// V = 1 (lengths 128..1024): 16 or 32 points per thread and two passes, i.e. ONE shared-memory exchange per transform.
-// These kernels are co-limited by HBM and by the load-store pipe (round 1: 0.70-0.84 of the copy bandwidth at 64-76 % LSU
-// utilisation with two exchanges); per element the pipe then carries 4 instead of 6 sixteen-byte accesses.
-#ifndef MHD_AXIS_BIG
-#define MHD_AXIS_BIG 0
-#endif
-template <int N, int V> struct AxisOcc {      // CTAs per SM the launch bounds ask for
-#ifndef MHD_AXIS_BIG_OCC
-#define MHD_AXIS_BIG_OCC 4
-#endif
-    static constexpr int value = (V == 1) ? ((227 * 1024) / (int)Tile<N, V>::SMEM > MHD_AXIS_BIG_OCC ? MHD_AXIS_BIG_OCC : (227 * 1024) / (int)Tile<N, V>::SMEM) : 1;
-};
-
-template <int N, bool INV, int V>
-__global__ void __launch_bounds__(Tile<N, V>::THREADS, AxisOcc<N, V>::value) fft_axis_kernel(AxisArgs a, const cplx* __restrict__ tw) {
+template <int N, bool INV>
+__global__ void __launch_bounds__(Tile<N>::THREADS) fft_axis_kernel(AxisArgs a, const cplx* __restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smraw[];
-    using PL = Plan<N, V>;
+    using PL = Plan<N>;
     const int tid = threadIdx.x, p = tid & 7, i = (tid >> 3) % PL::TP, g = tid / (8 * PL::TP);
     cplx* sm = reinterpret_cast<cplx*>(smraw) + (size_t)g * N * 8;
-    const int col = blockIdx.x * Tile<N, V>::COLS + g * 8 + p;
+    const int col = blockIdx.x * Tile<N>::COLS + g * 8 + p;
     const bool colok = col < a.inner;
     const long long outer = (long long)blockIdx.y + (long long)blockIdx.z * gridDim.y;
     if (outer >= a.nouter) return;           // uniform per CTA
@@ -54,38 +46,35 @@ __global__ void __launch_bounds__(Tile<N, V>::THREADS, AxisOcc<N, V>::value) fft
     for (int m = 0; m < PL::E / R0; ++m)
 #pragma unroll
         for (int q = 0; q < R0; ++q) {
-            const int c = compact_index(first_index<N, V>(i, m, q), N, a.nk_in);
+            const int c = compact_index(first_index<N>(i, m, q), N, a.nk_in);
             v[m * R0 + q] = (colok && c >= 0) ? in[(long long)c * a.in_row] : make_double2(0.0, 0.0);
         }
-#ifndef MHD_AXIS_COPYONLY      // (experiment: -DMHD_AXIS_COPYONLY measures the access pattern alone)
-    pencil_fft<N, INV, V>(v, sm, i, p, tw);
-#endif
+    pencil_fft<N, INV>(v, sm, i, p, tw);
     const double s = a.scale;
 #pragma unroll
     for (int m = 0; m < PL::E / RL; ++m)
 #pragma unroll
         for (int q = 0; q < RL; ++q) {
-            const int c = compact_index(last_index<N, V>(i, m, q), N, a.nk_out);
+            const int c = compact_index(last_index<N>(i, m, q), N, a.nk_out);
             if (colok && c >= 0) out[(long long)c * a.out_row] = make_double2(v[m * RL + q].x * s, v[m * RL + q].y * s);
         }
 }
 
 // ---- launchers -----------------------------------------------------------------------------
 template <int N, bool INV> static cudaError_t launch_axis_n(const AxisArgs& a, const cplx* tw, cudaStream_t st) {
-    constexpr int V = (MHD_AXIS_BIG && HasBigPlan<N>::value) ? 1 : 0;
     const long long outer = a.nouter;
     static DeviceOnce once;
     const int dev = device_slot();
     if (dev < 0) return cudaErrorInvalidDevice;
     if (!once.done[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(fft_axis_kernel<N, INV, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile<N, V>::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(fft_axis_kernel<N, INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile<N>::SMEM);
         if (e != cudaSuccess) return e;
         once.done[dev] = true;
     }
-    const unsigned tiles = (unsigned)((a.inner + Tile<N, V>::COLS - 1) / Tile<N, V>::COLS);
+    const unsigned tiles = (unsigned)((a.inner + Tile<N>::COLS - 1) / Tile<N>::COLS);
     unsigned gy = (unsigned)outer, gz = 1;
     while (gy > 65535u) { gz *= 2; gy = (unsigned)((outer + gz - 1) / gz); }
-    fft_axis_kernel<N, INV, V><<<dim3(tiles, gy, gz), Tile<N, V>::THREADS, Tile<N, V>::SMEM, st>>>(a, tw);
+    fft_axis_kernel<N, INV><<<dim3(tiles, gy, gz), Tile<N>::THREADS, Tile<N>::SMEM, st>>>(a, tw);
     count_launch();
     return cudaGetLastError();
 }

@@ -804,8 +804,8 @@ int mhd_fft_plan_create(mhd_fft_plan** out, int nx, int ny, int nz, int batch, v
     p->nx = nx; p->ny = ny; p->nz = nz; p->batch = batch; p->nxh = nx / 2 + 1; p->st = (cudaStream_t)stream;
     char* ws = (char*)workspace;
     p->twx = (double2*)(ws + L.twx); p->twy = (double2*)(ws + L.twy); p->twz = (double2*)(ws + L.twz); p->work = (double2*)(ws + L.work);
-    p->plane = planefft_supported(nx, ny) ? 1 : 0;
-    if (p->plane) {
+    p->plane = 0;              // default: three sweeps (faster on B200, see mhd_fft_plan_set_mode in mhd.h)
+    if (planefft_supported(nx, ny)) {
         const PlaneGeom g = plane_geom(nx);
         p->group = g.group; p->ring_slots = g.ring_slots; p->lag = g.lag; p->pitch = g.pitch;
         p->ring = (double2*)(ws + L.ring); p->counters = (unsigned*)(ws + L.counters);
@@ -825,6 +825,13 @@ int mhd_fft_plan_create(mhd_fft_plan** out, int nx, int ny, int nz, int batch, v
 }
 
 void mhd_fft_plan_destroy(mhd_fft_plan* p) { delete p; }
+
+int mhd_fft_plan_set_mode(mhd_fft_plan* p, int mode) {
+    if (!p || (mode != MHD_FFT_THREE_SWEEP && mode != MHD_FFT_PLANE_PIPELINE)) return MHD_EINVAL;
+    if (mode == MHD_FFT_PLANE_PIPELINE && !planefft_supported(p->nx, p->ny)) return MHD_EINVAL;
+    p->plane = (mode == MHD_FFT_PLANE_PIPELINE) ? 1 : 0;
+    return MHD_OK;
+}
 
 const char* mhd_fft_last_error(const mhd_fft_plan* p) { return p ? p->err : ""; }
 

@@ -28,6 +28,7 @@
 // [field][row][px] array (a row's inputs are all consumed before its outputs are written).
 #include "mhd_internal.h"
 #include "xteam.cuh"
+#include "bulk_copy.cuh"
 
 #ifndef MHD_XF_PREFETCH
 #define MHD_XF_PREFETCH 1
@@ -41,53 +42,42 @@ using namespace mhdfft;
 
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
-// ---- TMA bulk copy (cp.async.bulk, global -> shared) completing on an mbarrier ----
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
-                 "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "XF_WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra XF_DONE_%=;\n"
-        "bra XF_WAIT_%=;\n"
-        "XF_DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
+// threads per persistent CTA of the fused pass for N >= 256: 256 = 4 rows in flight per SM at N = 512 (8 warps, up to 255 registers), each with two
+// transforms in flight per thread (XPass2)
+#ifndef MHD_XF2_THREADS
+#define MHD_XF2_THREADS 256
+#endif
+template <int N> struct XCfg2 {
+    static constexpr int TP = Plan<N>::TP;
+    static constexpr int THREADS = (N >= 256) ? (MHD_XF2_THREADS / TP > 0 ? (MHD_XF2_THREADS / TP) * TP : TP) : 128;
+    static constexpr int TEAMS = THREADS / TP;
+    static constexpr int BUF = Padded::size(N);
+    static constexpr int NTW = XCfg<N>::NTW > 0 ? XCfg<N>::NTW : 1;
+    static constexpr size_t SMEM = sizeof(cplx) * ((size_t)2 * BUF * TEAMS + NTW);     // one exchange buffer per transform in flight
+};
 
 // PRUNED: nkx <= 3*TP (always true under the 2/3 rule), so the first-pass inputs q = 3, 4 are identically zero, the
-// split only needs k = i + TP*t with t <= 2, and the rows are staged through shared memory by TMA.
+// split only needs k = i + TP*t with t <= 2, and the rows are staged through shared memory by TMA: two staging areas per
+// team, one per field group (rho, mx, my, mz | Bx, By, Bz), each refilled for the team's next row as soon as it is consumed.
 template <int N, bool HYDRO, bool PRUNED>
-__global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs a, const cplx* __restrict__ tw) {
+__global__ void __launch_bounds__(XCfg2<N>::THREADS, 1) xfused_kernel(XFusedArgs a, const cplx* __restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smraw[];
     using PL = Plan<N>;
-    using CF = XCfg<N>;
+    using CF = XCfg2<N>;
     static_assert(PL::E == 8 && PL::radix(0) == 8, "fused x pass needs 8 points per thread and a radix-8 first pass");
     constexpr int TP = PL::TP, E = 8;
     constexpr int RL = PL::radix(PL::NP - 1);
-    constexpr int NIN = HYDRO ? 2 : 4, NOUT = HYDRO ? 5 : 6;
+    constexpr int NGRP = HYDRO ? 1 : 2;       // inverse: (rho,mx | my,mz) and (Bx,By | Bz,-)
+    constexpr int NFWD = 3;                   // forward: (ux,uy | uz,Txx) (Tyy,Tzz | Txy,Txz) (Tyz,Ex | Ey,Ez); hydro: (Tyz,- | -,-)
     const int team = threadIdx.x / TP, i = threadIdx.x % TP;
     cplx* const smbase = reinterpret_cast<cplx*>(smraw);
     cplx* const stw = smbase + (size_t)2 * CF::BUF * CF::TEAMS;
-    cplx* bufA = smbase + (size_t)team * 2 * CF::BUF;
-    cplx* bufB = bufA + CF::BUF;
+    cplx* const bufA = smbase + (size_t)team * 2 * CF::BUF;
+    cplx* const bufB = bufA + CF::BUF;
     const int nkx = a.nkx;
-    // TMA staging (PRUNED only): per team 2 buffers x 2 rows x px complex, and one mbarrier per buffer
-    cplx* const stage = stw + (CF::NTW > 0 ? CF::NTW : 1) + (size_t)team * 4 * a.px;
-    unsigned long long* const mbar = reinterpret_cast<unsigned long long*>(stw + (CF::NTW > 0 ? CF::NTW : 1) + (size_t)CF::TEAMS * 4 * a.px) + 2 * team;
+    // TMA staging (PRUNED only): per team 2 groups x 4 rows x px complex, and one mbarrier per group
+    cplx* const stage = stw + CF::NTW + (size_t)team * 8 * a.px;
+    unsigned long long* const mbar = reinterpret_cast<unsigned long long*>(stw + CF::NTW + (size_t)CF::TEAMS * 8 * a.px) + 2 * team;
     if (PRUNED && i == 0) { mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); }
     if (PRUNED) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 
@@ -96,7 +86,7 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
         int P = PL::radix(0);
 #pragma unroll
         for (int s = 1; s < PL::NP; ++s) {
-            const int R = PL::radix(s), off = CF::tw_offset(s);
+            const int R = PL::radix(s), off = XCfg<N>::tw_offset(s);
             for (int e = threadIdx.x; e < (R - 1) * P; e += blockDim.x) {
                 const int q = e / P + 1, k = e % P;
                 stw[off + e] = tw[k * q * (N / (P * R))];
@@ -107,23 +97,20 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
     __syncthreads();
 
     const long long row_stride = (long long)gridDim.x * CF::TEAMS;
-    const int pf_lines = (nkx * (int)sizeof(cplx) + 127) / 128;     // 128-byte lines per row (rows are 128-byte aligned)
     const unsigned row_bytes = (unsigned)nkx * (unsigned)sizeof(cplx);
-    (void)pf_lines;
 
-    // issue the TMA copies of field pair `pair` of row `r` into staging buffer (pair & 1): one thread per team
-    auto stage_pair = [&](long long r, int pair) {
-        const cplx* src = a.w2 + r * a.px + (long long)(2 * pair) * a.field_stride;
-        cplx* dst = stage + (size_t)(pair & 1) * 2 * a.px;
-        const bool two = pair < 3;
-        mbar_expect_tx(&mbar[pair & 1], two ? 2 * row_bytes : row_bytes);
-        bulk_g2s(dst, src, row_bytes, &mbar[pair & 1]);
-        if (two) bulk_g2s(dst + a.px, src + a.field_stride, row_bytes, &mbar[pair & 1]);
+    // issue the TMA copies of field group `grp` of row `r` into its staging area: one thread per team
+    auto stage_group = [&](long long r, int grp) {
+        const int nf = (grp == 0) ? 4 : 3;
+        const cplx* src = a.w2 + r * a.px + (long long)(4 * grp) * a.field_stride;
+        cplx* dst = stage + (size_t)grp * 4 * a.px;
+        mbar_expect_tx(&mbar[grp], (unsigned)nf * row_bytes);
+        for (int f = 0; f < nf; ++f) bulk_g2s(dst + (size_t)f * a.px, src + (long long)f * a.field_stride, row_bytes, &mbar[grp]);
     };
-    unsigned phase = 0;          // bit b = parity the next wait on mbar[b] expects
+    unsigned phase = 0;          // bit g = parity the next wait on mbar[g] expects
     if (PRUNED) {
         const long long row0 = (long long)blockIdx.x * CF::TEAMS + team;
-        if (i == 0 && row0 < a.nrows) { stage_pair(row0, 0); stage_pair(row0, 1); }
+        if (i == 0 && row0 < a.nrows) { stage_group(row0, 0); if (!HYDRO) stage_group(row0, 1); }
     }
 
     for (long long row = (long long)blockIdx.x * CF::TEAMS + team; row - team < a.nrows; row += row_stride) {
@@ -131,153 +118,114 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
         const bool ok = row < a.nrows;
         cplx* __restrict__ base = a.w2 + (ok ? row : 0) * a.px;
 
-#if MHD_XF_PREFETCH
-        if (!PRUNED && ok)
-            for (int f = 2; f < (HYDRO ? 4 : NFIELD); ++f)
-                for (int l = i; l < pf_lines; l += TP) prefetch_l1(reinterpret_cast<const char*>(base + (long long)f * a.field_stride) + 128 * l);
-#endif
-
         double inv[E], mx[E], my[E], mz[E], bx[E], by[E], bz[E];
 #pragma unroll
         for (int j = 0; j < E; ++j) { inv[j] = 1.0; mx[j] = 0.0; my[j] = 0.0; mz[j] = 0.0; bx[j] = 0.0; by[j] = 0.0; bz[j] = 0.0; }
 
-        // ---- inverse: field pairs (rho, mx) (my, mz) (Bx, By) (Bz, -) ----
-#pragma unroll 1
-        for (int pair = 0; pair < NIN; ++pair) {
-            const bool hasB = pair < 3;
-            cplx v[E];
+        // ---- inverse: two transforms at a time, (rho + i mx | my + i mz) then (Bx + i By | Bz) ----
+#pragma unroll
+        for (int grp = 0; grp < NGRP; ++grp) {
+            cplx va[E], vb[E];
+            // rows of this group: A0 + i A1 -> va, B0 + i B1 -> vb (B1 absent in the magnetic group)
+            const bool hasB1 = (grp == 0);
             if constexpr (PRUNED) {
-                const cplx* __restrict__ A = stage + (size_t)(pair & 1) * 2 * a.px;
-                const cplx* __restrict__ B = A + a.px;
-                if (ok) { mbar_wait(&mbar[pair & 1], (phase >> (pair & 1)) & 1u); phase ^= 1u << (pair & 1); }
+                const cplx* __restrict__ S0 = stage + (size_t)grp * 4 * a.px;
+                if (ok) { mbar_wait(&mbar[grp], (phase >> grp) & 1u); phase ^= 1u << grp; }
 #pragma unroll
                 for (int q = 0; q < E; ++q) {                 // first-pass input k = i + TP*q; q = 3, 4 lie in the pruned band
-                    if (q == 3 || q == 4) { v[q] = make_double2(0.0, 0.0); continue; }
+                    if (q == 3 || q == 4) { va[q] = make_double2(0.0, 0.0); vb[q] = make_double2(0.0, 0.0); continue; }
                     const int k = i + TP * q;
                     const bool lo = (q < 3) && k < nkx, hi = (q > 4) && (N - k) < nkx;
                     const int idx = (q < 3) ? k : N - k;
-                    cplx x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
-                    if (ok && (lo || hi)) { x = A[idx]; if (hasB) y = B[idx]; }
-                    if (k == 0) { x.y = 0.0; y.y = 0.0; }                               // self-conjugate mode: Im ignored
-                    v[q] = (q < 3) ? make_double2(x.x - y.y, x.y + y.x) : make_double2(x.x + y.y, y.x - x.y);
+                    cplx x0 = make_double2(0.0, 0.0), x1 = x0, y0 = x0, y1 = x0;
+                    if (ok && (lo || hi)) {
+                        x0 = S0[idx]; x1 = S0[a.px + idx]; y0 = S0[2 * a.px + idx];
+                        if (hasB1) y1 = S0[3 * a.px + idx];
+                    }
+                    if (k == 0) { x0.y = 0.0; x1.y = 0.0; y0.y = 0.0; y1.y = 0.0; }                       // self-conjugate mode: Im ignored
+                    va[q] = (q < 3) ? make_double2(x0.x - x1.y, x0.y + x1.x) : make_double2(x0.x + x1.y, x1.x - x0.y);
+                    vb[q] = (q < 3) ? make_double2(y0.x - y1.y, y0.y + y1.x) : make_double2(y0.x + y1.y, y1.x - y0.y);
                 }
             } else {
-                const cplx* __restrict__ A = base + (long long)(2 * pair) * a.field_stride;
-                const cplx* __restrict__ B = hasB ? A + a.field_stride : A;
+                const cplx* __restrict__ G0 = base + (long long)(4 * grp) * a.field_stride;
 #pragma unroll
                 for (int q = 0; q < E; ++q) {                 // first-pass input k = i + TP*q
                     const int k = i + TP * q;
                     const bool lo = k < nkx, hi = (N - k) < nkx;
                     const int idx = lo ? k : N - k;
-                    cplx x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
-                    if (ok && (lo || hi)) { x = A[idx]; if (hasB) y = B[idx]; }
-                    if (k == 0 || 2 * k == N) { x.y = 0.0; y.y = 0.0; }                 // self-conjugate modes: Im ignored
+                    cplx x0 = make_double2(0.0, 0.0), x1 = x0, y0 = x0, y1 = x0;
+                    if (ok && (lo || hi)) {
+                        x0 = G0[idx]; x1 = G0[a.field_stride + idx]; y0 = G0[2 * a.field_stride + idx];
+                        if (hasB1) y1 = G0[3 * a.field_stride + idx];
+                    }
+                    if (k == 0 || 2 * k == N) { x0.y = 0.0; x1.y = 0.0; y0.y = 0.0; y1.y = 0.0; }       // self-conjugate modes: Im ignored
                     // lo: A + iB;   hi (and not lo): conj(A) + i conj(B)
-                    v[q] = lo ? make_double2(x.x - y.y, x.y + y.x) : make_double2(x.x + y.y, y.x - x.y);
+                    va[q] = lo ? make_double2(x0.x - x1.y, x0.y + x1.x) : make_double2(x0.x + x1.y, x1.x - x0.y);
+                    vb[q] = lo ? make_double2(y0.x - y1.y, y0.y + y1.x) : make_double2(y0.x + y1.y, y1.x - y0.y);
                 }
             }
-            XPass<N, true, 0, 1>::run(v, bufA, bufB, i, team, stw);
-            if (odd_exchanges<N>()) { cplx* t = bufA; bufA = bufB; bufB = t; }
+            XPass2<N, true, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
             if constexpr (PRUNED) {
-                // staging buffer (pair & 1) is free again: the team has passed a barrier since reading it (a one-thread
-                // team needs none).  Refill it with pair + 2 of this row, or with the team's next row.
+                // the staging area of this group is free again: the team has passed a barrier since reading it (a one-thread
+                // team needs none).  Refill it with the same group of the team's next row.
                 if constexpr (PL::NP == 1 && TP > 1) team_sync<TP>(team);
-                if (i == 0 && ok) {
-                    if (pair + 2 < NIN) stage_pair(row, pair + 2);
-                    else if (row + row_stride < a.nrows) stage_pair(row + row_stride, pair + 2 - NIN);
-                }
+                if (i == 0 && ok && row + row_stride < a.nrows) stage_group(row + row_stride, grp);
             }
             const double s = a.scale;
             // last-pass outputs: register m*RL + q holds x = i + TP*m + q*(N/RL) = i + TP*(m + q*(E/RL))
-            switch (pair) {
-                case 0:
 #pragma unroll
-                    for (int m = 0; m < E / RL; ++m)
+            for (int m = 0; m < E / RL; ++m)
 #pragma unroll
-                        for (int q = 0; q < RL; ++q) { inv[m + q * (E / RL)] = v[m * RL + q].x * s; mx[m + q * (E / RL)] = v[m * RL + q].y * s; }
-                    break;
-                case 1:
-#pragma unroll
-                    for (int m = 0; m < E / RL; ++m)
-#pragma unroll
-                        for (int q = 0; q < RL; ++q) { my[m + q * (E / RL)] = v[m * RL + q].x * s; mz[m + q * (E / RL)] = v[m * RL + q].y * s; }
-                    break;
-                case 2:
-#pragma unroll
-                    for (int m = 0; m < E / RL; ++m)
-#pragma unroll
-                        for (int q = 0; q < RL; ++q) { bx[m + q * (E / RL)] = v[m * RL + q].x * s; by[m + q * (E / RL)] = v[m * RL + q].y * s; }
-                    break;
-                default:
-#pragma unroll
-                    for (int m = 0; m < E / RL; ++m)
-#pragma unroll
-                        for (int q = 0; q < RL; ++q) bz[m + q * (E / RL)] = v[m * RL + q].x * s;
-                    break;
-            }
+                for (int q = 0; q < RL; ++q) {
+                    const int j = m + q * (E / RL), r = m * RL + q;
+                    if (grp == 0) { inv[j] = va[r].x * s; mx[j] = va[r].y * s; my[j] = vb[r].x * s; mz[j] = vb[r].y * s; }
+                    else { bx[j] = va[r].x * s; by[j] = va[r].y * s; bz[j] = vb[r].x * s; }
+                }
         }
 #pragma unroll
         for (int j = 0; j < E; ++j) inv[j] = ok ? 1.0 / inv[j] : 1.0;
 
-        // ---- forward: product pairs (ux,uy) (uz,Txx) (Tyy,Tzz) (Txy,Txz) (Tyz,Ex) (Ey,Ez) ----
+        // ---- forward: four products (two transforms) at a time ----
 #pragma unroll 1
-        for (int fp = 0; fp < NOUT; ++fp) {
-            cplx v[E];
-            int ida, idb;
+        for (int it = 0; it < NFWD; ++it) {
+            cplx va[E], vb[E];
+            int ida, idb, idc, idd;            // output fields of va.re, va.im, vb.re, vb.im (-1: none)
             // keep the compiler from hoisting the (loop-invariant) products out of this rolled loop and spilling them
 #pragma unroll
             for (int j = 0; j < E; ++j) {
                 asm volatile("" : "+d"(inv[j]));
                 if constexpr (!HYDRO) asm volatile("" : "+d"(bx[j]), "+d"(by[j]), "+d"(bz[j]));
             }
-            switch (fp) {
+            switch (it) {
                 case 0:
-                    ida = P_UX; idb = P_UY;
+                    ida = P_UX; idb = P_UY; idc = P_UZ; idd = P_TXX;
 #pragma unroll
-                    for (int j = 0; j < E; ++j) v[j] = make_double2(mx[j] * inv[j], my[j] * inv[j]);
+                    for (int j = 0; j < E; ++j) {
+                        va[j] = make_double2(mx[j] * inv[j], my[j] * inv[j]);
+                        vb[j] = make_double2(mz[j] * inv[j], mx[j] * (mx[j] * inv[j]) + 0.5 * (bx[j] * bx[j] + by[j] * by[j] + bz[j] * bz[j]) - bx[j] * bx[j]);
+                    }
                     break;
                 case 1:
-                    ida = P_UZ; idb = P_TXX;
-#pragma unroll
-                    for (int j = 0; j < E; ++j)
-                        v[j] = make_double2(mz[j] * inv[j], mx[j] * (mx[j] * inv[j]) + 0.5 * (bx[j] * bx[j] + by[j] * by[j] + bz[j] * bz[j]) - bx[j] * bx[j]);
-                    break;
-                case 2:
-                    ida = P_TYY; idb = P_TZZ;
+                    ida = P_TYY; idb = P_TZZ; idc = P_TXY; idd = P_TXZ;
 #pragma unroll
                     for (int j = 0; j < E; ++j) {
                         const double b2h = 0.5 * (bx[j] * bx[j] + by[j] * by[j] + bz[j] * bz[j]);
-                        v[j] = make_double2(my[j] * (my[j] * inv[j]) + b2h - by[j] * by[j], mz[j] * (mz[j] * inv[j]) + b2h - bz[j] * bz[j]);
+                        va[j] = make_double2(my[j] * (my[j] * inv[j]) + b2h - by[j] * by[j], mz[j] * (mz[j] * inv[j]) + b2h - bz[j] * bz[j]);
+                        vb[j] = make_double2(mx[j] * (my[j] * inv[j]) - bx[j] * by[j], mx[j] * (mz[j] * inv[j]) - bx[j] * bz[j]);
                     }
                     break;
-                case 3:
-                    ida = P_TXY; idb = P_TXZ;
-#pragma unroll
-                    for (int j = 0; j < E; ++j) v[j] = make_double2(mx[j] * (my[j] * inv[j]) - bx[j] * by[j], mx[j] * (mz[j] * inv[j]) - bx[j] * bz[j]);
-                    break;
-                case 4:
-                    ida = P_TYZ; idb = HYDRO ? -1 : P_EX;
-#pragma unroll
-                    for (int j = 0; j < E; ++j)
-                        v[j] = make_double2(my[j] * (mz[j] * inv[j]) - by[j] * bz[j], HYDRO ? 0.0 : (my[j] * inv[j]) * bz[j] - (mz[j] * inv[j]) * by[j]);
-                    break;
                 default:
-                    ida = P_EY; idb = P_EZ;
+                    ida = P_TYZ; idb = HYDRO ? -1 : P_EX; idc = HYDRO ? -1 : P_EY; idd = HYDRO ? -1 : P_EZ;
 #pragma unroll
-                    for (int j = 0; j < E; ++j)
-                        v[j] = make_double2((mz[j] * inv[j]) * bx[j] - (mx[j] * inv[j]) * bz[j], (mx[j] * inv[j]) * by[j] - (my[j] * inv[j]) * bx[j]);
+                    for (int j = 0; j < E; ++j) {
+                        va[j] = make_double2(my[j] * (mz[j] * inv[j]) - by[j] * bz[j], HYDRO ? 0.0 : (my[j] * inv[j]) * bz[j] - (mz[j] * inv[j]) * by[j]);
+                        vb[j] = HYDRO ? make_double2(0.0, 0.0)
+                                      : make_double2((mz[j] * inv[j]) * bx[j] - (mx[j] * inv[j]) * bz[j], (mx[j] * inv[j]) * by[j] - (my[j] * inv[j]) * bx[j]);
+                    }
                     break;
             }
-#if MHD_XF_PREFETCH
-            if (!PRUNED && fp == NOUT - 2 && row + row_stride < a.nrows) {       // next row of this team: first two field pairs
-                const cplx* nb = a.w2 + (row + row_stride) * a.px;
-                for (int f = 0; f < (HYDRO ? 2 : 4); ++f)
-                    for (int l = i; l < pf_lines; l += TP) prefetch_l1(reinterpret_cast<const char*>(nb + (long long)f * a.field_stride) + 128 * l);
-            }
-#endif
-            // first-pass input register q must hold x = i + TP*q: that is how v was filled (j = q)
-            XPass<N, false, 0, 1>::run(v, bufA, bufB, i, team, stw);
-            if (odd_exchanges<N>()) { cplx* t = bufA; bufA = bufB; bufB = t; }
+            // first-pass input register q must hold x = i + TP*q: that is how va, vb were filled (j = q)
+            XPass2<N, false, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
             // Hermitian split: A[k] = (Z[k] + conj Z[N-k])/2, B[k] = (Z[k] - conj Z[N-k])/(2i), k = i + TP*t < nkx.
             // Z[k] is this thread's own last-pass output; only Z[N-k] (held by slot (TP-i)%TP) crosses threads.
             // last-pass register m*RL + q holds index i + TP*(m + q*(E/RL)); publish those some k' = N-k can ask for.
@@ -287,12 +235,17 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
                 for (int q = 0; q < RL; ++q) {
                     const int t = m + q * (E / RL);            // index i + TP*t
                     if (PRUNED && t < 5) continue;                   // N - k > N - nkx >= 5*TP
-                    if (t >= 1 && (TP * (t + 1) > N - nkx)) bufA[N - (i + TP * t)] = v[m * RL + q];   // index range [TP*t, TP*t+TP) meets [N-nkx+1, N)
+                    if (t >= 1 && (TP * (t + 1) > N - nkx)) {        // index range [TP*t, TP*t+TP) meets [N-nkx+1, N)
+                        bufA[N - (i + TP * t)] = va[m * RL + q];
+                        bufB[N - (i + TP * t)] = vb[m * RL + q];
+                    }
                 }
             team_sync<TP>(team);
             if (ok) {
                 cplx* __restrict__ oa = base + (long long)ida * a.field_stride;
                 cplx* __restrict__ ob = base + (long long)(idb < 0 ? 0 : idb) * a.field_stride;
+                cplx* __restrict__ oc = base + (long long)(idc < 0 ? 0 : idc) * a.field_stride;
+                cplx* __restrict__ od = base + (long long)(idd < 0 ? 0 : idd) * a.field_stride;
 #pragma unroll
                 for (int m = 0; m < E / RL; ++m)
 #pragma unroll
@@ -300,14 +253,18 @@ __global__ void __launch_bounds__(XCfg<N>::THREADS, 1) xfused_kernel(XFusedArgs 
                         const int t = m + q * (E / RL);
                         const int k = i + TP * t;
                         if (t <= (PRUNED ? 2 : E / 2) && k < nkx) {
-                            const cplx zk = v[m * RL + q];
+                            const cplx zk = va[m * RL + q];
                             const cplx zm = (k == 0) ? zk : bufA[k];      // Z[N-k], published at position N - index (unpadded: conflict-free both ways)
                             oa[k] = make_double2(0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y));
                             if (idb >= 0) ob[k] = make_double2(0.5 * (zk.y + zm.y), 0.5 * (zm.x - zk.x));
+                            const cplx yk = vb[m * RL + q];
+                            const cplx ym = (k == 0) ? yk : bufB[k];
+                            if (idc >= 0) oc[k] = make_double2(0.5 * (yk.x + ym.x), 0.5 * (yk.y - ym.y));
+                            if (idd >= 0) od[k] = make_double2(0.5 * (yk.y + ym.y), 0.5 * (ym.x - yk.x));
                         }
                     }
             }
-            { cplx* t = bufA; bufA = bufB; bufB = t; }
+            team_sync<TP>(team);              // the split reads are done before the next transform's first exchange writes the buffers
         }
     }
 }
@@ -335,8 +292,8 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
     const int team = threadIdx.x / TP, i = threadIdx.x % TP;
     cplx* const smbase = reinterpret_cast<cplx*>(smraw);
     cplx* const stw = smbase + (size_t)2 * CF::BUF * RC::TEAMS;
-    cplx* bufA = smbase + (size_t)team * 2 * CF::BUF;
-    cplx* bufB = bufA + CF::BUF;
+    cplx* const bufA = smbase + (size_t)team * 2 * CF::BUF;
+    cplx* const bufB = bufA + CF::BUF;
     const int nkx = a.nkx;
     {
         int P = PL::radix(0);
@@ -351,70 +308,86 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
         }
     }
     __syncthreads();
+    // a team takes TWO row pairs per iteration (two transforms in flight per thread, XPass2): the kernel is latency-bound
     const long long npairs = (a.nrows + 1) / 2;
+    const long long nunits = (npairs + 1) / 2;
     const long long stride = (long long)gridDim.x * RC::TEAMS;
-    for (long long pr = (long long)blockIdx.x * RC::TEAMS + team; pr - team < npairs; pr += stride) {
-        const bool ok = pr < npairs;
-        const long long r0 = ok ? 2 * pr : 0;
-        cplx* __restrict__ A = a.spec + r0 * a.spec_pitch;
-        cplx* __restrict__ B = A + a.spec_pitch;
-        double* __restrict__ ra = a.real + r0 * a.real_pitch;
-        double* __restrict__ rb = ra + a.real_pitch;
-        cplx v[E];
+    for (long long u = (long long)blockIdx.x * RC::TEAMS + team; u - team < nunits; u += stride) {
+        const bool oka = 2 * u < npairs, okb = 2 * u + 1 < npairs;
+        const long long r0 = oka ? 4 * u : 0, r1 = okb ? 4 * u + 2 : 0;
+        cplx* __restrict__ A0 = a.spec + r0 * a.spec_pitch;
+        cplx* __restrict__ A1 = A0 + a.spec_pitch;
+        cplx* __restrict__ B0 = a.spec + r1 * a.spec_pitch;
+        cplx* __restrict__ B1 = B0 + a.spec_pitch;
+        double* __restrict__ ra0 = a.real + r0 * a.real_pitch;
+        double* __restrict__ ra1 = ra0 + a.real_pitch;
+        double* __restrict__ rb0 = a.real + r1 * a.real_pitch;
+        double* __restrict__ rb1 = rb0 + a.real_pitch;
+        cplx va[E], vb[E];
         if constexpr (INV) {
 #pragma unroll
             for (int q = 0; q < E; ++q) {                 // first-pass input k = i + TP*q
                 const int k = i + TP * q;
                 const bool lo = k < nkx, hi = (N - k) < nkx;
                 const int idx = lo ? k : N - k;
-                cplx x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
-                if (ok && (lo || hi)) { x = A[idx]; y = B[idx]; }
-                if (k == 0 || 2 * k == N) { x.y = 0.0; y.y = 0.0; }                 // self-conjugate modes: Im ignored
-                v[q] = lo ? make_double2(x.x - y.y, x.y + y.x) : make_double2(x.x + y.y, y.x - x.y);
+                cplx x0 = make_double2(0.0, 0.0), x1 = x0, y0 = x0, y1 = x0;
+                if (lo || hi) {
+                    if (oka) { x0 = A0[idx]; x1 = A1[idx]; }
+                    if (okb) { y0 = B0[idx]; y1 = B1[idx]; }
+                }
+                if (k == 0 || 2 * k == N) { x0.y = 0.0; x1.y = 0.0; y0.y = 0.0; y1.y = 0.0; }   // self-conjugate modes: Im ignored
+                va[q] = lo ? make_double2(x0.x - x1.y, x0.y + x1.x) : make_double2(x0.x + x1.y, x1.x - x0.y);
+                vb[q] = lo ? make_double2(y0.x - y1.y, y0.y + y1.x) : make_double2(y0.x + y1.y, y1.x - y0.y);
             }
-            XPass<N, true, 0, 1>::run(v, bufA, bufB, i, team, stw);
-            if (odd_exchanges<N>()) { cplx* t = bufA; bufA = bufB; bufB = t; }
+            XPass2<N, true, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
             const double s = a.scale;
-            if (ok) {
 #pragma unroll
-                for (int m = 0; m < E / RL; ++m)
+            for (int m = 0; m < E / RL; ++m)
 #pragma unroll
-                    for (int q = 0; q < RL; ++q) {
-                        const int x = i + TP * (m + q * (E / RL));
-                        ra[x] = v[m * RL + q].x * s;
-                        rb[x] = v[m * RL + q].y * s;
-                    }
-            }
+                for (int q = 0; q < RL; ++q) {
+                    const int x = i + TP * (m + q * (E / RL));
+                    if (oka) { ra0[x] = va[m * RL + q].x * s; ra1[x] = va[m * RL + q].y * s; }
+                    if (okb) { rb0[x] = vb[m * RL + q].x * s; rb1[x] = vb[m * RL + q].y * s; }
+                }
         } else {
 #pragma unroll
-            for (int q = 0; q < E; ++q) v[q] = ok ? make_double2(ra[i + TP * q], rb[i + TP * q]) : make_double2(0.0, 0.0);
-            XPass<N, false, 0, 1>::run(v, bufA, bufB, i, team, stw);
-            if (odd_exchanges<N>()) { cplx* t = bufA; bufA = bufB; bufB = t; }
+            for (int q = 0; q < E; ++q) {
+                va[q] = oka ? make_double2(ra0[i + TP * q], ra1[i + TP * q]) : make_double2(0.0, 0.0);
+                vb[q] = okb ? make_double2(rb0[i + TP * q], rb1[i + TP * q]) : make_double2(0.0, 0.0);
+            }
+            XPass2<N, false, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
+            // Hermitian split: only Z[N-k] crosses threads (see the fused kernel)
 #pragma unroll
             for (int m = 0; m < E / RL; ++m)
 #pragma unroll
                 for (int q = 0; q < RL; ++q) {
                     const int t = m + q * (E / RL);
-                    if (t >= 1 && (TP * (t + 1) > N - nkx)) bufA[N - (i + TP * t)] = v[m * RL + q];
+                    if (t >= 1 && (TP * (t + 1) > N - nkx)) { bufA[N - (i + TP * t)] = va[m * RL + q]; bufB[N - (i + TP * t)] = vb[m * RL + q]; }
                 }
             team_sync<TP>(team);
             const double s = 0.5 * a.scale;
-            if (ok) {
 #pragma unroll
-                for (int m = 0; m < E / RL; ++m)
+            for (int m = 0; m < E / RL; ++m)
 #pragma unroll
-                    for (int q = 0; q < RL; ++q) {
-                        const int t = m + q * (E / RL);
-                        const int k = i + TP * t;
-                        if (t <= E / 2 && k < nkx) {
-                            const cplx zk = v[m * RL + q];
+                for (int q = 0; q < RL; ++q) {
+                    const int t = m + q * (E / RL);
+                    const int k = i + TP * t;
+                    if (t <= E / 2 && k < nkx) {
+                        if (oka) {
+                            const cplx zk = va[m * RL + q];
                             const cplx zm = (k == 0) ? zk : bufA[k];
-                            A[k] = make_double2(s * (zk.x + zm.x), s * (zk.y - zm.y));
-                            B[k] = make_double2(s * (zk.y + zm.y), s * (zm.x - zk.x));
+                            A0[k] = make_double2(s * (zk.x + zm.x), s * (zk.y - zm.y));
+                            A1[k] = make_double2(s * (zk.y + zm.y), s * (zm.x - zk.x));
+                        }
+                        if (okb) {
+                            const cplx zk = vb[m * RL + q];
+                            const cplx zm = (k == 0) ? zk : bufB[k];
+                            B0[k] = make_double2(s * (zk.x + zm.x), s * (zk.y - zm.y));
+                            B1[k] = make_double2(s * (zk.y + zm.y), s * (zm.x - zk.x));
                         }
                     }
-            }
-            { cplx* t = bufA; bufA = bufB; bufB = t; }
+                }
+            team_sync<TP>(team);
         }
     }
 }
@@ -557,7 +530,7 @@ template <int N> static cudaError_t launch_xrows_n(bool inverse, const RowArgs& 
             if (e != cudaSuccess) return e;
             once.done[dev] = true;
         }
-        const long long groups = ((a.nrows + 1) / 2 + RC::TEAMS - 1) / RC::TEAMS;
+        const long long groups = (((a.nrows + 1) / 2 + 1) / 2 + RC::TEAMS - 1) / RC::TEAMS;   // two row pairs per team iteration
         const long long cap = (long long)sms * 8;             // persistent; more CTAs than can be resident simply queue
         const unsigned blocks = (unsigned)(groups < cap ? groups : cap);
         if (inverse) xrows_kernel<N, true><<<blocks, RC::THREADS, RC::SMEM, st>>>(a, tw);
@@ -580,11 +553,11 @@ template <int N> static cudaError_t launch_xfused_n(const XFusedArgs& a, int hyd
     if constexpr (Plan<N>::E != 8) {
         return cudaErrorInvalidValue;
     } else {
-        using CF = XCfg<N>;
+        using CF = XCfg2<N>;
         constexpr size_t kMaxSmem = 227 * 1024;
-        // staged (TMA) rows need 2 buffers x 2 rows x px complex per team + the mbarriers
+        // staged (TMA) rows need 2 groups x 4 rows x px complex per team + the mbarriers
         const bool pruned = a.nkx <= 3 * CF::TP;
-        const size_t smem = CF::SMEM + (pruned ? sizeof(cplx) * (size_t)CF::TEAMS * 4 * a.px + 16 * (size_t)CF::TEAMS : 0);
+        const size_t smem = CF::SMEM + (pruned ? sizeof(cplx) * (size_t)CF::TEAMS * 8 * a.px + 16 * (size_t)CF::TEAMS : 0);
         if (smem > kMaxSmem) return cudaErrorInvalidValue;
         static DeviceOnce once;
         const int dev = device_slot();

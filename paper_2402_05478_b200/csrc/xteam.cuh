@@ -15,6 +15,10 @@
 #ifndef MHD_XF_THREADS
 #define MHD_XF_THREADS 384
 #endif
+// the same choice for the two-transform passes (XPass2), where one set of twiddles serves both transforms
+#ifndef MHD_XF2_TW
+#define MHD_XF2_TW 2
+#endif
 
 namespace mhd {
 using namespace mhdfft;
@@ -118,6 +122,91 @@ struct XPass {
                 }
             if constexpr (SINGLE) team_sync<TP>(team);
             XPass<N, INV, S + 1, P * R, SINGLE>::run(v, sm1, sm0, i, team, stw);
+        }
+    }
+};
+
+
+// Two independent transforms per thread (va, vb), pass by pass in lock step: the twiddles of a pass are formed once and
+// applied to both, one team barrier serves both exchanges, and the two butterflies give every warp two independent
+// instruction streams (the fused x pass is latency-bound: 12 warps per SM cannot cover the FP64 and shared-memory
+// latencies of a single stream).  One exchange buffer per transform (smA, smB), two barriers per exchange.
+template <int N, bool INV, int S, int P>
+struct XPass2 {
+    using PL = Plan<N>;
+    static constexpr int R = PL::radix(S);
+    static constexpr int E = PL::E;
+    static constexpr int TP = PL::TP;
+    static constexpr bool LAST = (S == PL::NP - 1);
+    __device__ __forceinline__ static void run(cplx (&va)[E], cplx (&vb)[E], cplx* smA, cplx* smB, int i, int team, const cplx* __restrict__ stw) {
+#pragma unroll
+        for (int m = 0; m < E / R; ++m) {
+            const int b = i + TP * m;
+            const int k = b & (P - 1);
+            if constexpr (S > 0) {
+                const cplx* __restrict__ t = stw + XCfg<N>::tw_offset(S) + k;
+                if constexpr (R == 8 && (MHD_XF2_TW == 2 || (MHD_XF2_TW == 3 && P >= 32) || (MHD_XF2_TW == 1 && P >= 32))) {
+                    cplx w1 = t[0], w2, w3, w4, w5, w6, w7;
+                    if (INV) w1.y = -w1.y;
+                    if constexpr (MHD_XF2_TW == 3) {      // w, w^2, w^4 from the table, four products of depth 1
+                        w2 = t[P]; w4 = t[3 * P];
+                        if (INV) { w2.y = -w2.y; w4.y = -w4.y; }
+                        w3 = cmul(w1, w2); w5 = cmul(w1, w4); w6 = cmul(w2, w4); w7 = cmul(w3, w4);
+                    } else {                              // everything from w (depth 3)
+                        w2 = cmul(w1, w1); w3 = cmul(w2, w1); w4 = cmul(w2, w2);
+                        w5 = cmul(w4, w1); w6 = cmul(w3, w3); w7 = cmul(w4, w3);
+                    }
+                    va[m * R + 1] = cmul(va[m * R + 1], w1); vb[m * R + 1] = cmul(vb[m * R + 1], w1);
+                    va[m * R + 2] = cmul(va[m * R + 2], w2); vb[m * R + 2] = cmul(vb[m * R + 2], w2);
+                    va[m * R + 3] = cmul(va[m * R + 3], w3); vb[m * R + 3] = cmul(vb[m * R + 3], w3);
+                    va[m * R + 4] = cmul(va[m * R + 4], w4); vb[m * R + 4] = cmul(vb[m * R + 4], w4);
+                    va[m * R + 5] = cmul(va[m * R + 5], w5); vb[m * R + 5] = cmul(vb[m * R + 5], w5);
+                    va[m * R + 6] = cmul(va[m * R + 6], w6); vb[m * R + 6] = cmul(vb[m * R + 6], w6);
+                    va[m * R + 7] = cmul(va[m * R + 7], w7); vb[m * R + 7] = cmul(vb[m * R + 7], w7);
+                } else {
+#pragma unroll
+                    for (int q = 1; q < R; ++q) {
+                        cplx w = t[(q - 1) * P];
+                        if (INV) w.y = -w.y;
+                        va[m * R + q] = cmul(va[m * R + q], w);
+                        vb[m * R + q] = cmul(vb[m * R + q], w);
+                    }
+                }
+            }
+            bfly<R, INV>(&va[m * R]);
+            bfly<R, INV>(&vb[m * R]);
+            if constexpr (!LAST) {
+                if constexpr (P == 1) {            // first pass: j = R*b, element j + q
+                    const int j = b * R, pj = xpad(j);
+#pragma unroll
+                    for (int q = 0; q < R; ++q) {
+                        const int o = (R == 8) ? pj + q : xpad(j + q);
+                        smA[o] = va[m * R + q]; smB[o] = vb[m * R + q];
+                    }
+                } else {
+                    const int j = (b - k) * R + k, pj = xpad(j);
+#pragma unroll
+                    for (int q = 0; q < R; ++q) {
+                        const int o = (P % 8 == 0) ? pj + q * (P + P / 8) : xpad(j + q * P);
+                        smA[o] = va[m * R + q]; smB[o] = vb[m * R + q];
+                    }
+                }
+            }
+        }
+        if constexpr (!LAST) {
+            constexpr int Rn = PL::radix(S + 1);
+            team_sync<TP>(team);
+            const int pi = xpad(i);
+#pragma unroll
+            for (int m = 0; m < E / Rn; ++m)
+#pragma unroll
+                for (int q = 0; q < Rn; ++q) {
+                    const int D = TP * m + q * (N / Rn);
+                    const int o = (D % 8 == 0) ? pi + D + D / 8 : xpad(i + D);
+                    va[m * Rn + q] = smA[o]; vb[m * Rn + q] = smB[o];
+                }
+            team_sync<TP>(team);
+            XPass2<N, INV, S + 1, P * R>::run(va, vb, smA, smB, i, team, stw);
         }
     }
 };

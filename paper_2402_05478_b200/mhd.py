@@ -17,13 +17,14 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = 0, -1, -2, -3, -4, -5
 AB2, RK4 = 0, 1
 FLAG_HYDRO, FLAG_NO_DEALIAS, FLAG_FORCING = 1, 2, 4
 FLAG_UNFUSED_X, FLAG_NO_GRAPH, FLAG_FUSED_ZSTAGE = 8, 16, 32
+FFT_THREE_SWEEP, FFT_PLANE_PIPELINE = 0, 1
 
 EXPORTS = [
     "mhd_workspace_bytes", "mhd_create", "mhd_destroy", "mhd_set_fields", "mhd_set_fields_host", "mhd_set_box",
     "mhd_set_forcing", "mhd_set_forcing_host", "mhd_step",
     "mhd_state_bytes", "mhd_get_state", "mhd_set_state",
     "mhd_get_fields", "mhd_get_fields_host", "mhd_diagnostics", "mhd_strerror", "mhd_last_error",
-    "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy", "mhd_fft_last_error",
+    "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy", "mhd_fft_last_error", "mhd_fft_plan_set_mode",
     "mhd_launch_count", "mhd_profile_kernel_count", "mhd_profile_kernel_name", "mhd_profile_begin", "mhd_profile_end",
     "mhd_measure_peaks",
 ]
@@ -83,6 +84,7 @@ def lib():
         L.mhd_fft_c2r.argtypes = [_vp, _vp, _vp]
         L.mhd_fft_plan_destroy.argtypes = [_vp]
         L.mhd_fft_plan_destroy.restype = None
+        L.mhd_fft_plan_set_mode.argtypes = [_vp, C.c_int]
         L.mhd_fft_last_error.restype = C.c_char_p
         L.mhd_fft_last_error.argtypes = [_vp]
         L.mhd_launch_count.restype = C.c_longlong
@@ -322,7 +324,7 @@ class FftPlan:
     def stream(self):
         return self._stream
 
-    def __init__(self, nx, ny, nz, batch, stream=None, device="cuda:0"):
+    def __init__(self, nx, ny, nz, batch, stream=None, device="cuda:0", mode=FFT_THREE_SWEEP):
         torch = _torch()
         L = lib()
         self.nx, self.ny, self.nz, self.batch = int(nx), int(ny), int(nz), int(batch)
@@ -343,6 +345,14 @@ class FftPlan:
             raise MhdError(rc, "mhd_fft_plan_create")
         self.real_shape = (self.batch, self.nz, self.ny, self.nx)
         self.spec_shape = (self.batch, self.nz, self.ny, self.nx // 2 + 1)
+        if mode != FFT_THREE_SWEEP:
+            self.set_mode(mode)
+
+    def set_mode(self, mode):
+        """FFT_THREE_SWEEP (default) or FFT_PLANE_PIPELINE (x and y passes through an L2-resident ring; square planes 64..512)"""
+        rc = lib().mhd_fft_plan_set_mode(self._h, int(mode))
+        if rc != OK:
+            raise MhdError(rc, "mhd_fft_plan_set_mode")
 
     def r2c(self, real, out=None):
         torch = _torch()

@@ -20,12 +20,12 @@ def gpu():
     return mhd
 
 
-def check(gpu, ref, shape, batch, tol=2e-14):
+def check(gpu, ref, shape, batch, tol=2e-14, mode=0):
     import torch
     nz, ny, nx = shape
     rng = np.random.default_rng(nx * 7 + ny * 3 + nz)
     a = rng.uniform(-1, 1, size=(batch, nz, ny, nx))
-    plan = gpu.FftPlan(nx, ny, nz, batch)
+    plan = gpu.FftPlan(nx, ny, nz, batch, mode=mode)
     da = torch.from_numpy(a).cuda()
     spec = plan.r2c(da)
     want = ref.fft_r2c(a)
@@ -58,20 +58,22 @@ def test_batched_3d_and_2d(gpu, ref, shape, batch):
 @pytest.mark.parametrize("shape,batch", [((8, 512, 512), 3), ((12, 256, 256), 3), ((24, 64, 64), 1), ((8, 128, 128), 1),
                                          ((1, 512, 512), 1), ((48, 128, 128), 5)])
 def test_plane_pipelined_xy_pass_against_the_oracle(gpu, ref, shape, batch):
-    """square (x,y) planes of 64..512 take the persistent plane-pipelined kernel (x and y passes meet in an L2-resident ring,
-    planefft_kernel.cu): plane counts that do not fill the last group, a single plane, more groups than ring slots; twice in
-    a row on the same plan (the ring and the counters are reused)."""
-    check(gpu, ref, shape, batch)
-    check(gpu, ref, shape, batch)
+    """MHD_FFT_PLANE_PIPELINE: square (x,y) planes of 64..512 through the persistent plane-pipelined kernel (x and y passes
+    meet in an L2-resident ring, planefft_kernel.cu): plane counts that do not fill the last group, a single plane, more
+    groups than ring slots; twice in a row (the ring and the counters are reused); other shapes are refused."""
+    check(gpu, ref, shape, batch, mode=gpu.FFT_PLANE_PIPELINE)
+    check(gpu, ref, shape, batch, mode=gpu.FFT_PLANE_PIPELINE)
+    with pytest.raises(gpu.MhdError):
+        gpu.FftPlan(32, 16, 8, 1, mode=gpu.FFT_PLANE_PIPELINE)
 
 
-@pytest.mark.parametrize("n", [256, 512, 768])
-def test_round_trip_at_bench_sizes(gpu, n):
+@pytest.mark.parametrize("n,mode", [(256, 0), (512, 0), (768, 0), (256, 1), (512, 1)])
+def test_round_trip_at_bench_sizes(gpu, n, mode):
     """config 5 sizes the oracle cannot finish in seconds: round trip and Parseval hold at any size."""
     import torch
     batch = 7 if n <= 256 else 2
     a = torch.from_numpy(inputs.config5_batch(n, batch)).cuda()
-    plan = gpu.FftPlan(n, n, n, batch)
+    plan = gpu.FftPlan(n, n, n, batch, mode=mode)
     spec = plan.r2c(a)
     back = plan.c2r(spec)
     assert float(torch.linalg.norm(back - a) / torch.linalg.norm(a)) <= 1e-14
