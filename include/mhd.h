@@ -50,8 +50,7 @@ enum {
      * through this ABI.  Nothing in the library reads the environment. */
     MHD_FLAG_UNFUSED_X = 8u,      /* x C2R, real-space products and x R2C as three kernels through real arrays, instead of the
                                      fused x pass (the plan that lengths 3*2^a would need if the fused pass did not cover them) */
-    MHD_FLAG_NO_GRAPH = 16u,      /* mhd_step always enqueues its kernels one by one (no CUDA-graph replay) */
-    MHD_FLAG_FUSED_ZSTAGE = 32u   /* last forward FFT axis and the integrator stage in one kernel (the flux spectra are never stored) */
+    MHD_FLAG_NO_GRAPH = 16u       /* mhd_step always enqueues its kernels one by one (no CUDA-graph replay) */
 };
 
 /* mean values are volume averages <.> = (1/N) sum over the grid */
@@ -168,8 +167,8 @@ long long mhd_launch_count(void);
  * eagerly with a CUDA-event pair around every launch (on the context's stream); mhd_profile_end
  * synchronises, fills counts[i] (launches) and ms[i] (summed device time) for the
  * mhd_profile_kernel_count() kernel classes named by mhd_profile_kernel_name(i) -- in hot-path
- * order: z inverse, y inverse, x C2R, products, x R2C, fused x pass, y forward, z forward, stage, fused z-forward +
- * stage -- and switches profiling off.  Both arrays are HOST memory of that length. */
+ * order: z inverse, y inverse, x C2R, products, x R2C, fused x pass, y forward, z forward, stage -- and switches
+ * profiling off.  Both arrays are HOST memory of that length. */
 int mhd_profile_kernel_count(void);
 const char* mhd_profile_kernel_name(int i);
 int mhd_profile_begin(mhd_ctx* ctx);

@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmhd_b200.so")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["fft_kernels.cu", "xfused_kernel.cu", "planefft_kernel.cu", "zstage_kernel.cu", "mhd_kernels.cu", "peaks_kernel.cu",
+SOURCES = ["fft_kernels.cu", "xfused_kernel.cu", "planefft_kernel.cu", "mhd_kernels.cu", "peaks_kernel.cu",
            "mhd_api.cu"]
 HEADERS = ["fft_core.cuh", "xteam.cuh", "bulk_copy.cuh", "mhd_internal.h"]
 

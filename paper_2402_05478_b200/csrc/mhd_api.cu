@@ -19,8 +19,8 @@ namespace {
 constexpr int kMaxShell = 2048;
 
 // kernel classes timed by mhd_profile_begin / mhd_profile_end, in hot-path order
-enum { K_Z_INV = 0, K_Y_INV, K_X_C2R, K_PRODUCTS, K_X_R2C, K_XFUSED, K_Y_FWD, K_Z_FWD, K_STAGE, K_ZSTAGE, K_NCLASS };
-const char* const kClassNames[K_NCLASS] = {"fft_z_inv", "fft_y_inv", "fft_x_c2r", "products", "fft_x_r2c", "x_fused", "fft_y_fwd", "fft_z_fwd", "stage", "z_fwd_stage"};
+enum { K_Z_INV = 0, K_Y_INV, K_X_C2R, K_PRODUCTS, K_X_R2C, K_XFUSED, K_Y_FWD, K_Z_FWD, K_STAGE, K_NCLASS };
+const char* const kClassNames[K_NCLASS] = {"fft_z_inv", "fft_y_inv", "fft_x_c2r", "products", "fft_x_r2c", "x_fused", "fft_y_fwd", "fft_z_fwd", "stage"};
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -108,7 +108,6 @@ struct mhd_ctx {
     cudaGraphExec_t graph;     // one steady-state step (AB2 non-first / RK4), replayed by mhd_step
     int graph_ready;
     long long graph_launches;  // kernels inside the captured step
-    int zfuse;                 // z forward pass fused with the stage (zstage_kernel.cu) available for this nz
     int xfuse;                 // fused x pass available for this nx (and not disabled by MHD_NO_XFUSE)
     int profiling;             // mhd_profile_begin: eager steps with CUDA events around every kernel
     std::vector<cudaEvent_t>* prof_ev;   // [K_NCLASS] start/stop pairs
@@ -208,21 +207,21 @@ cudaError_t inverse_fields(mhd_ctx* c, const double2* src, int nf, double* real_
     return timed(c, K_X_C2R, [&] { return launch_fft_rows(g.nx, true, r, c->twx, c->st); });
 }
 
-cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst, bool y_only = false);
+cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst);
 
 // real fields -> compact spectral fields (x real-to-complex, y forward, z forward), unnormalised
-cudaError_t forward_fields(mhd_ctx* c, const double* real_in, int nf, double2* dst, bool y_only = false) {
+cudaError_t forward_fields(mhd_ctx* c, const double* real_in, int nf, double2* dst) {
     const Geometry& g = c->g;
     cudaError_t e;
     RowArgs r;
     r.spec = c->W2; r.real = const_cast<double*>(real_in); r.spec_pitch = g.px; r.real_pitch = g.nx;
     r.nrows = (long long)nf * g.nz * g.ny; r.nkx = g.nkx; r.scale = 1.0;
     if ((e = timed(c, K_X_R2C, [&] { return launch_fft_rows(g.nx, false, r, c->twx, c->st); })) != cudaSuccess) return e;
-    return forward_yz(c, nf, dst, y_only);
+    return forward_yz(c, nf, dst);
 }
 
 // W2 half-spectrum rows -> compact spectral fields (y forward, z forward)
-cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst, bool y_only) {
+cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst) {
     const Geometry& g = c->g;
     cudaError_t e;
     {
@@ -233,7 +232,7 @@ cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst, bool y_only) {
         a.inner = g.px; a.nk_in = g.ny; a.nk_out = g.nky; a.scale = 1.0;
         if ((e = timed(c, K_Y_FWD, [&] { return launch_fft_axis(g.ny, false, a, c->twy, c->st); })) != cudaSuccess) return e;
     }
-    if (g.nz > 1 && !y_only) {
+    if (g.nz > 1) {
         AxisArgs a;
         a.in = c->W1; a.out = dst; a.nouter = nf;
         a.in_outer = g.w1field; a.out_outer = g.fieldc;
@@ -248,28 +247,22 @@ cudaError_t forward_yz(mhd_ctx* c, int nf, double2* dst, bool y_only) {
 cudaError_t rhs_stage(mhd_ctx* c, int mode) {
     const Geometry& g = c->g;
     cudaError_t e;
-    const bool zf = c->zfuse != 0;
     if (c->xfuse) {   // x inverse + products + x forward in one kernel, in place on W2
         if ((e = inverse_zy(c, c->S, c->hydro ? 4 : NFIELD)) != cudaSuccess) return e;
         XFusedArgs x;
         x.w2 = c->W2; x.field_stride = g.w2field; x.nrows = (long long)g.nz * g.ny; x.px = g.px; x.nkx = g.nkx;
         x.scale = 1.0 / (double)g.npts;
         if ((e = timed(c, K_XFUSED, [&] { return launch_xfused(g.nx, x, c->hydro, c->twx, c->st); })) != cudaSuccess) return e;
-        if ((e = forward_yz(c, c->hydro ? 9 : NPROD, c->G, zf)) != cudaSuccess) return e;
+        if ((e = forward_yz(c, c->hydro ? 9 : NPROD, c->G)) != cudaSuccess) return e;
     } else {
         if ((e = inverse_fields(c, c->S, c->hydro ? 4 : NFIELD, c->Rf)) != cudaSuccess) return e;
         if ((e = timed(c, K_PRODUCTS, [&] { return launch_products(c->Rf, c->Rg, g.npts, c->hydro, c->st); })) != cudaSuccess) return e;
-        if ((e = forward_fields(c, c->Rg, c->hydro ? 9 : NPROD, c->G, zf)) != cudaSuccess) return e;
+        if ((e = forward_fields(c, c->Rg, c->hydro ? 9 : NPROD, c->G)) != cudaSuccess) return e;
     }
     StageArgs s;
     s.g = spec_geom(g); s.S = c->S; s.G = c->G; s.H = c->H; s.Acc = c->Acc;
     s.nu = c->nu; s.eta = c->eta; s.cs2 = c->cs * c->cs; s.dt = c->dt; s.mode = mode; s.hydro = c->hydro;
     s.F = c->have_forcing ? c->Fh : nullptr; s.kfx = c->kf[0]; s.kfy = c->kf[1]; s.kfz = c->kf[2];
-    if (zf) {   // last forward axis and the stage in one kernel: the flux spectra G are never stored
-        ZStageArgs z;
-        z.W1 = c->W1; z.w1field = g.w1field; z.inner = (long long)g.nky * g.px; z.st = s;
-        return timed(c, K_ZSTAGE, [&] { return launch_zstage(g.nz, z, c->twz, c->st); });
-    }
     return timed(c, K_STAGE, [&] { return launch_stage(s, c->st); });
 }
 
@@ -360,7 +353,7 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     if (integrator != MHD_AB2 && integrator != MHD_RK4) return MHD_EINVAL;
     if (!(nu >= 0.0) || !(eta >= 0.0) || !(cs >= 0.0) || !(dt > 0.0)) return MHD_EINVAL;
     if (!isfinite(nu) || !isfinite(eta) || !isfinite(cs) || !isfinite(dt)) return MHD_EINVAL;
-    if (flags & ~(MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS | MHD_FLAG_FORCING | MHD_FLAG_UNFUSED_X | MHD_FLAG_NO_GRAPH | MHD_FLAG_FUSED_ZSTAGE))
+    if (flags & ~(MHD_FLAG_HYDRO | MHD_FLAG_NO_DEALIAS | MHD_FLAG_FORCING | MHD_FLAG_UNFUSED_X | MHD_FLAG_NO_GRAPH))
         return MHD_EINVAL;
     const Layout L = make_layout(g, integrator, flags);
     if (!workspace || workspace_bytes < L.total || ((size_t)workspace & 255u)) return MHD_EINVAL;
@@ -373,7 +366,6 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     c->device = owning_device(workspace);
     DeviceGuard guard(c->device);
     c->xfuse = use_xfuse(nx, flags);
-    c->zfuse = nz > 1 && zstage_supported(nz) && (flags & MHD_FLAG_FUSED_ZSTAGE);
     c->prof_ev = new (std::nothrow) std::vector<cudaEvent_t>[K_NCLASS];
     if (!c->prof_ev) { delete c; return MHD_ENOMEM; }
     c->twx = (double2*)(c->ws + L.twx); c->twy = (double2*)(c->ws + L.twy); c->twz = (double2*)(c->ws + L.twz);

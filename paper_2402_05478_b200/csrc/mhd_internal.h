@@ -88,16 +88,6 @@ struct StageArgs {
     int hydro;
 };
 
-// last forward axis (z) fused with the stage (zstage_kernel.cu): reads the 12 (9 hydro) flux fields on [z][nky][px]
-struct ZStageArgs {
-    const double2* W1;        // [field][nz][inner]
-    long long w1field;        // complex elements per field = nz * inner
-    long long inner;          // nky * px
-    StageArgs st;             // st.G is unused
-};
-bool zstage_supported(int nz);
-cudaError_t launch_zstage(int nz, const ZStageArgs& a, const double2* tw, cudaStream_t st);
-
 cudaError_t launch_products(const double* f, double* g, long long npts, int hydro, cudaStream_t st);
 cudaError_t launch_stage(const StageArgs& a, cudaStream_t st);
 cudaError_t launch_momentum(const double* rho, const double* ux, const double* uy, const double* uz, double* m,

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmhd_b200.so")
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = 0, -1, -2, -3, -4, -5
 AB2, RK4 = 0, 1
 FLAG_HYDRO, FLAG_NO_DEALIAS, FLAG_FORCING = 1, 2, 4
-FLAG_UNFUSED_X, FLAG_NO_GRAPH, FLAG_FUSED_ZSTAGE = 8, 16, 32
+FLAG_UNFUSED_X, FLAG_NO_GRAPH = 8, 16
 FFT_THREE_SWEEP, FFT_PLANE_PIPELINE = 0, 1
 
 EXPORTS = [

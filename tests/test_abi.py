@@ -106,7 +106,7 @@ def test_library_has_no_hidden_dispatch_and_no_per_process_device_state():
         assert not re.search(r"static\s+(int\s+sms|bool\s+attr_done)", text), f
     internal = open(os.path.join(csrc, "mhd_internal.h")).read()
     assert "struct DeviceOnce" in internal and "kMaxDevices" in internal
-    for f in ("fft_kernels.cu", "xfused_kernel.cu", "zstage_kernel.cu"):
+    for f in ("fft_kernels.cu", "xfused_kernel.cu", "planefft_kernel.cu"):
         text = open(os.path.join(csrc, f)).read()
         assert text.count("cudaFuncSetAttribute") > 0 and "once.done[dev]" in text, f
 

@@ -153,40 +153,16 @@ def test_paper_diagnostics_on_config1_and_closed_forms(gpu, ref):
     assert abs(d["enstrophy"] - 4 * 3 * 0.49) <= 1e-12 and abs(d["rayleigh_q"] - 4.0) <= 1e-12
 
 
-@pytest.mark.parametrize("integrator,hydro", [(0, False), (1, False), (0, True)])
-def test_fused_z_forward_stage_kernel_matches_oracle(gpu, ref, integrator, hydro):
-    """the fused z-forward + stage kernel (zstage_kernel.cu, MHD_FLAG_FUSED_ZSTAGE): same results as the oracle,
-    with forcing and a stretched box, Euler start + steady AB2 (graph replay) or RK4."""
-    import torch
-    shape = (32, 16, 64)
-    f = inputs.smooth_random_state(64, 16, 32, seed=41, hydro=hydro)
-    force = [0.05 * np.cos(np.arange(64) * TWO_PI / 64)[None, None, :] * np.ones(shape), np.zeros(shape), 0.02 * np.ones(shape)]
-    flags = gpu.FLAG_FORCING | gpu.FLAG_FUSED_ZSTAGE | (gpu.FLAG_HYDRO if hydro else 0)
-    o, g = both(gpu, ref, shape, f, 3e-3, 2e-3, 1.1, 1e-3, integrator=integrator, flags=flags, box=(TWO_PI, 3.0, 5.0), force=force)
-    launches0 = gpu.launch_count()
-    o.step(1); g.step(1)
-    got = [t.cpu().numpy() for t in g.get_fields()]
-    want = o.get_fields()
-    assert max(rel(got[0:1], want[0:1]), rel(got[1:4], want[1:4])) <= PER_STEP
-    o.step(8); g.step(8)
-    got = [t.cpu().numpy() for t in g.get_fields()]
-    want = o.get_fields()
-    assert max(rel(got[0:1], want[0:1]), rel(got[1:4], want[1:4])) <= 1e-12
-    if not hydro:
-        assert rel(got[4:7], want[4:7]) <= 1e-12
-    assert gpu.launch_count() > launches0
-
-
 def test_execution_plan_flags_do_not_change_the_result(gpu, ref):
     """MHD_FLAG_NO_GRAPH is bit-identical to the default plan (same kernels, launched one by one); MHD_FLAG_UNFUSED_X (x C2R,
-    products kernel, x R2C through real arrays) and MHD_FLAG_FUSED_ZSTAGE agree with it to roundoff and with the oracle at
-    the per-step bar.  Nothing is selected through the environment."""
+    products kernel, x R2C through real arrays) agrees with it to roundoff and with the oracle at the per-step bar.
+    Nothing is selected through the environment."""
     import torch
     cfg = inputs.config1()
     dev = [torch.from_numpy(a).cuda() for a in cfg.arrays()]
     res = {}
-    for name, fl in (("default", 0), ("nograph", gpu.FLAG_NO_GRAPH), ("unfused", gpu.FLAG_UNFUSED_X), ("zstage", gpu.FLAG_FUSED_ZSTAGE),
-                     ("all", gpu.FLAG_NO_GRAPH | gpu.FLAG_UNFUSED_X | gpu.FLAG_FUSED_ZSTAGE)):
+    for name, fl in (("default", 0), ("nograph", gpu.FLAG_NO_GRAPH), ("unfused", gpu.FLAG_UNFUSED_X),
+                     ("all", gpu.FLAG_NO_GRAPH | gpu.FLAG_UNFUSED_X)):
         s = gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, flags=fl)
         s.set_fields(*dev); s.step(9)
         res[name] = [t.cpu().numpy() for t in s.get_fields()]
@@ -195,7 +171,7 @@ def test_execution_plan_flags_do_not_change_the_result(gpu, ref):
     o = ref.RefSolver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt)
     o.set_fields(*cfg.arrays()); o.step(9)
     want = o.get_fields()
-    for name in ("unfused", "zstage", "all"):
+    for name in ("unfused", "all"):
         assert rel(res[name], res["default"]) <= 1e-13, name
         assert rel(res[name], want) <= 1e-12, name
     with pytest.raises(gpu.MhdError):
