@@ -473,6 +473,11 @@ def fft_sweep_rows(sizes, dev, peak, reps=5, cufft=True):
                "r2c_eff_gbs": (fr + fc) / 1e9 / (t_r2c * 1e-3), "c2r_eff_gbs": (fr + fc) / 1e9 / (t_c2r * 1e-3)}
         row["r2c_frac"] = row["r2c_eff_gbs"] / peak
         row["c2r_frac"] = row["c2r_eff_gbs"] / peak
+        if n in (64, 128, 256, 512):     # the 2-sweep plan mode (x and y passes through an L2-resident ring), measured beside the default
+            plan.set_mode(mhd.FFT_PLANE_PIPELINE)
+            row["plane_pipeline_r2c_ms"] = timed(lambda: plan.r2c(a, out=spec))
+            row["plane_pipeline_c2r_ms"] = timed(lambda: plan.c2r(spec, out=back))
+            plan.set_mode(mhd.FFT_THREE_SWEEP)
         plan.close()
         del plan, back
         if cufft:

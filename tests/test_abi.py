@@ -117,3 +117,8 @@ def test_peaks_probe_rejects_bad_arguments(lib):
     assert lib.mhd_measure_peaks(None, 1 << 23, None, C.byref(f), C.byref(s)) == mhd.EINVAL
     assert lib.mhd_measure_peaks(C.c_void_p(256), 16, None, C.byref(f), C.byref(s)) == mhd.EINVAL
     assert lib.mhd_fft_last_error(None) == b""
+    assert lib.mhd_fft_plan_set_mode(None, 0) == mhd.EINVAL
+    # the plane pipeline needs a ring + counters in the plan workspace only for square planes of 64..512
+    assert lib.mhd_fft_workspace_bytes(512, 512, 8, 1) > lib.mhd_fft_workspace_bytes(512, 256, 8, 1) * 2 - (1 << 20)
+    ring = lib.mhd_fft_workspace_bytes(256, 256, 8, 1) - (16 * 256 * 3 + 16 * 129 * 256 * 8)
+    assert 15e6 < ring < 30e6                        # 5 slots of about 4 MB

@@ -43,6 +43,21 @@ def test_algorithmic_bytes_2d_hydro_has_no_z_pass():
     assert b["x_fused"] == (4 + 9) * 256 * 86 * 16
 
 
+def test_xfused_onchip_model_matches_the_design_derivation():
+    """per row 10 transforms of 3 radix-8 passes of 64 butterflies (56 FP64 instructions + 28 twiddle
+    instructions on passes 2 and 3) + 35 per grid point; two exchanges of 2 x 16 B per point, 7 staged rows, 6 split pairs."""
+    g = bench.geometry(512, 512, 512)
+    dp, smem = bench.xfused_onchip_model(g)
+    rows = 512 * 512
+    assert dp == rows * (10 * 64 * (56 * 3 + 28 * 2) + 35 * 512)
+    assert smem == rows * (10 * 2 * 2 * 16 * 512 + 7 * 16 * 171 + 6 * 2 * 16 * 171)
+    # the floors they imply at the ceilings measured on B200 (34.1 TFLOP/s, 36.5 TB/s) bracket the HBM floor from above
+    alu_ms, smem_ms, hbm_ms = dp * 2 / 34.1e12 * 1e3, smem / 36.5e12 * 1e3, bench.algorithmic_bytes(g)["x_fused"] / 6542.1e9 * 1e3
+    assert 2.3 < alu_ms < 2.6 and 2.6 < smem_ms < 2.9 and 2.0 < hbm_ms < 2.2
+    dph, _ = bench.xfused_onchip_model(bench.geometry(256, 256, 1), hydro=True)
+    assert dph == 256 * (7 * 32 * (56 * 3 + 28 * 2) + 35 * 256)      # log8(256) rounds to 3 passes; 2 inverse + 5 forward transforms
+
+
 def test_parse_clock_samples():
     text = "\n".join([
         "0, 345, 1965, 180.1, 0x0000000000000000, Not Active, Not Active, Not Active, Not Active",

@@ -93,6 +93,7 @@ def test_config1_one_step_and_full_run(gpu, ref):
     o, g, err1 = run_both(gpu, ref, cfg, 1)
     assert err1 <= PER_STEP, err1
     o, g, err = run_both(gpu, ref, cfg, cfg.steps)
+    print(f"config 1 (32^3, {cfg.steps} steps): one step {err1:.2e}, end of run {err:.2e}")
     assert err <= END_OF_RUN, err
     assert err <= 1e-12          # in fact roundoff-level: no amplification over 20 smooth steps
     check_diag(g.diagnostics(20), o.diagnostics(20), 20)
@@ -160,6 +161,7 @@ def test_config2_kelvin_helmholtz_256(gpu, ref):
     o, g, err1 = run_both(gpu, ref, cfg, 1)
     assert err1 <= PER_STEP, err1
     o, g, err = run_both(gpu, ref, cfg, cfg.steps, check_every=500)
+    print(f"config 2 (256^2 KH, {cfg.steps} steps): one step {err1:.2e}, worst of the 500-step checkpoints {err:.2e}")
     assert err <= END_OF_RUN, err
     check_diag(g.diagnostics(), o.diagnostics())
 
@@ -170,6 +172,7 @@ def test_config3_orszag_tang_128(gpu, ref):
     o, g, err1 = run_both(gpu, ref, cfg, 1)
     assert err1 <= PER_STEP, err1
     o, g, err = run_both(gpu, ref, cfg, steps)
+    print(f"config 3 (128^3 OT, {steps} steps): one step {err1:.2e}, end of run {err:.2e}")
     assert err <= END_OF_RUN, err
     check_diag(g.diagnostics(64), o.diagnostics(64), 64)
 
