@@ -331,7 +331,8 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
             const long long un = u + stride;
             if (2 * un < npairs) {
                 const char* nsrc = reinterpret_cast<const char*>(a.spec + 4 * un * a.spec_pitch);
-                const long long bytes = 4 * a.spec_pitch * (long long)sizeof(cplx);
+                const long long left = a.nrows - 4 * un;                                   // rows that exist from there on
+                const long long bytes = (left < 4 ? left : 4) * a.spec_pitch * (long long)sizeof(cplx);
                 for (long long o = (long long)i * 128; o < bytes; o += (long long)TP * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(nsrc + o));
             }
         }
