@@ -6,41 +6,34 @@
 // eq. (2) PAPER.md:41 (rho u u + (B^2/2) I - B B), eq. (4) PAPER.md:47 (u x B), u = m/rho for the
 // viscous term; "products formed in real space" PAPER.md:78.
 //
-// Design (round-1 ncu of the first version: 255 registers, 8 warps/SM, 79 % of cycles without an
-// eligible warp, a third of the stalls on the row loads; see profiles/r01_summary.md):
+// Design (history and measurements: DESIGN.md §6, profiles/r02_experiments.md):
 //   * persistent CTAs, one per SM, of TEAMS independent teams; a TEAM of TP = N/8 threads owns one
-//     (z,y) row at a time (N = 512: 64 threads = 2 warps, 6 teams = 12 warps per SM).  Teams
-//     synchronise among themselves only (named barrier, or __syncwarp when a team fits a warp), so the
-//     FP64 phase of one team overlaps the shared-memory exchange of another.
+//     (z,y) row at a time (N = 512: 64 threads = 2 warps, 4 teams = 8 warps per SM, up to 255 registers).
+//     Teams synchronise among themselves only (named barrier, or __syncwarp when a team fits a warp).
 //   * two real fields share one complex transform (Z = A + iB) both ways.  Every thread keeps 8
 //     grid points x = i + TP*j of the 7 fields in registers: the inverse transform's last pass
 //     leaves exactly the set the forward transform's first pass consumes, so the products are
 //     thread-local.
-//   * between passes the data is exchanged through two alternating team-private padded buffers, so one
-//     barrier per exchange suffices; all shared-memory indices are a per-thread base plus
-//     compile-time offsets.
-//   * twiddles are read from per-pass shared tables laid out [leg][k] (conflict-free / broadcast).
+//   * TWO transforms are in flight per thread (XPass2): (rho+i mx | my+i mz), (Bx+i By | Bz) inverse and three pairs of
+//     product pairs forward.  Round 1 (12 warps/SM, one dependent stream each) was latency-bound: 53 % FP64 / 66 % LSU
+//     utilisation, and neither pipe's instruction count moved the time.  Two independent streams per warp, one set of
+//     twiddles and one barrier for both took it from 5.5 to 4.6 ms at 512^3 (LSU 72 % busy); four at once in the inverse
+//     half gains nothing more (a round of four costs what two rounds of two do: throughput-bound now).
+//   * between passes the data is exchanged through one team-private padded buffer per transform in flight; all
+//     shared-memory indices are a per-thread base plus compile-time offsets.
+//   * twiddles: w of a pass from a per-pass shared table laid out [leg][k], w^2..w^7 by multiplication.
 //   * the Hermitian split after a forward transform needs Z[N-k] only: 3 of the 8 outputs go through
 //     shared memory, Z[k] is already in the thread's own registers.
-//   * the rows of the next field pairs (and of the team's next row) are pulled into L1 with
-//     prefetch.global.L1 while the current transform runs, so the row loads hit L1.
+//   * the 7 input rows of a team's NEXT row are staged into shared memory by TMA (cp.async.bulk + mbarrier) while the
+//     current row is transformed, one staging area per field group.
 // HBM traffic: reads 7 rows of nkx complex, writes 12 rows of nkx complex, in place in the same
 // [field][row][px] array (a row's inputs are all consumed before its outputs are written).
 #include "mhd_internal.h"
 #include "xteam.cuh"
 #include "bulk_copy.cuh"
 
-#ifndef MHD_XF_PREFETCH
-#define MHD_XF_PREFETCH 1
-#endif
-// MHD_XF_THREADS (xteam.cuh): threads per persistent CTA for N >= 256 (a multiple of 128): 384 = 6 rows in flight per SM at N = 512
-// MHD_XF_TWCHAIN (xteam.cuh): the kernel is bound by shared-memory wavefronts (80 % of the LSU data pipe), not FP64 (43 %): 2 is
-// fastest (B200, 512^3).
-
 namespace mhd {
 using namespace mhdfft;
-
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // threads per persistent CTA of the fused pass for N >= 256: 256 = 4 rows in flight per SM at N = 512 (8 warps, up to 255 registers), each with two
 // transforms in flight per thread (XPass2)

@@ -12,9 +12,6 @@
 // 2 = every pass, 3 = table reads while the table row is one broadcast wavefront (P < 32), else w, w^2, w^4 + 4 products.
 #define MHD_XF_TWCHAIN 2
 #endif
-#ifndef MHD_XF_THREADS
-#define MHD_XF_THREADS 384
-#endif
 // the same choice for the two-transform passes (XPass2), where one set of twiddles serves both transforms
 #ifndef MHD_XF2_TW
 #define MHD_XF2_TW 2
@@ -25,8 +22,6 @@ using namespace mhdfft;
 
 template <int N> struct XCfg {
     static constexpr int TP = Plan<N>::TP;                      // threads per row
-    static constexpr int THREADS = (N >= 256) ? (MHD_XF_THREADS / TP) * TP : 128;   // whole teams only
-    static constexpr int TEAMS = THREADS / TP;                  // rows in flight per CTA
     static constexpr int BUF = Padded::size(N);                 // complex elements per exchange buffer
     // number of twiddle-table entries: sum over passes s >= 1 of (R_s - 1) * P_s
     __host__ __device__ static constexpr int tw_offset(int s) {  // first entry of pass s
@@ -35,7 +30,6 @@ template <int N> struct XCfg {
         return off;
     }
     static constexpr int NTW = tw_offset(Plan<N>::NP);
-    static constexpr size_t SMEM = sizeof(cplx) * ((size_t)2 * BUF * TEAMS + (NTW > 0 ? NTW : 1));
 };
 
 template <int TP> __device__ __forceinline__ void team_sync(int team) {
@@ -210,8 +204,5 @@ struct XPass2 {
         }
     }
 };
-
-// number of exchanges of one transform (decides which buffer the next exchange uses)
-template <int N> __device__ __forceinline__ constexpr bool odd_exchanges() { return ((Plan<N>::NP - 1) & 1) != 0; }
 
 }  // namespace mhd
