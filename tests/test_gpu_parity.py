@@ -302,7 +302,8 @@ def test_config4_512_sampled_parity_against_the_oracle_on_the_shared_grid(gpu, r
 
 
 @pytest.mark.parametrize("integrator", [0, 1])
-@pytest.mark.parametrize("shape", [(8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024), (8, 8, 768), (8, 768, 8)])
+@pytest.mark.parametrize("shape", [(8, 8, 512), (8, 512, 8), (512, 8, 8), (8, 8, 1024), (8, 1024, 8), (1024, 8, 8), (8, 8, 768), (8, 768, 8),
+                                   (768, 8, 8), (8, 8, 256), (8, 8, 64)])
 def test_full_band_state_through_every_pruned_index_path(gpu, ref, shape, integrator):
     """Production-length axes with O(1) energy in EVERY mode (white noise under a smooth envelope, rho in [0.7, 1.3]):
     the modes next to the 2/3 cut (index 170 kept / 171 dropped at 512), the zero-filled band of the
