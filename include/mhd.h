@@ -26,8 +26,9 @@
  * Pointers named *_dev are DEVICE pointers, *_host are HOST pointers (pinned memory makes the
  * copies asynchronous, pageable memory works too).  Every call returns MHD_OK or a negative code;
  * nothing throws, aborts or prints.  Invalid arguments are rejected before any launch.  A context
- * is not thread-safe; distinct contexts are independent.  Results are bit-reproducible run to run
- * (no floating-point atomics).
+ * is not thread-safe; distinct contexts are independent, also on different devices of one process: every
+ * call makes the device that owns the context's workspace current for its own duration and restores the caller's.
+ * Results are bit-reproducible run to run (no floating-point atomics).
  */
 #ifndef MHD_H
 #define MHD_H
@@ -49,7 +50,7 @@ enum {
      * covered by the same parity tests); they exist so that every kernel of the library can be reached, tested and timed
      * through this ABI.  Nothing in the library reads the environment. */
     MHD_FLAG_UNFUSED_X = 8u,      /* x C2R, real-space products and x R2C as three kernels through real arrays, instead of the
-                                     fused x pass (the plan that lengths 3*2^a would need if the fused pass did not cover them) */
+                                     fused x pass (the plan that nx = 3*2^a always uses: the fused pass needs 8 points per thread) */
     MHD_FLAG_NO_GRAPH = 16u       /* mhd_step always enqueues its kernels one by one (no CUDA-graph replay) */
 };
 
