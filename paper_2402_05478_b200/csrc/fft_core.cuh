@@ -15,6 +15,11 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#ifndef MHD_AXIS_TWCHAIN
+// twiddles of a radix-4/8 pass of the strided-axis kernels: 1 = w from the table, w^2..w^7 by multiplication; 0 = all from the table
+#define MHD_AXIS_TWCHAIN 1
+#endif
+
 namespace mhdfft {
 
 typedef double2 cplx;
@@ -156,11 +161,25 @@ struct Pass {
             const int b = i + TP * m;
             const int k = b & (P - 1);
             if constexpr (S > 0) {
+                if constexpr (MHD_AXIS_TWCHAIN && (R == 8 || R == 4)) {
+                    // one table read per butterfly, the other powers by multiplication (depth <= 3, a few ulp): the strided-axis
+                    // kernels are co-limited by the load-store pipe, and 7 twiddle reads per butterfly were 18 % of its wavefronts
+                    cplx w1 = __ldg(&tw[k * (N / (P * R))]);
+                    if (INV) w1.y = -w1.y;
+                    const cplx w2 = cmul(w1, w1), w3 = cmul(w2, w1);
+                    v[m * R + 1] = cmul(v[m * R + 1], w1); v[m * R + 2] = cmul(v[m * R + 2], w2); v[m * R + 3] = cmul(v[m * R + 3], w3);
+                    if constexpr (R == 8) {
+                        const cplx w4 = cmul(w2, w2), w5 = cmul(w4, w1), w6 = cmul(w3, w3), w7 = cmul(w4, w3);
+                        v[m * R + 4] = cmul(v[m * R + 4], w4); v[m * R + 5] = cmul(v[m * R + 5], w5);
+                        v[m * R + 6] = cmul(v[m * R + 6], w6); v[m * R + 7] = cmul(v[m * R + 7], w7);
+                    }
+                } else {
 #pragma unroll
-                for (int q = 1; q < R; ++q) {
-                    cplx w = __ldg(&tw[k * q * (N / (P * R))]);
-                    if (INV) w.y = -w.y;
-                    v[m * R + q] = cmul(v[m * R + q], w);
+                    for (int q = 1; q < R; ++q) {
+                        cplx w = __ldg(&tw[k * q * (N / (P * R))]);
+                        if (INV) w.y = -w.y;
+                        v[m * R + q] = cmul(v[m * R + q], w);
+                    }
                 }
             }
             bfly<R, INV>(&v[m * R]);
