@@ -222,6 +222,7 @@ __global__ void __launch_bounds__(XCfg2<N>::THREADS, 1) xfused_kernel(XFusedArgs
             // Hermitian split: A[k] = (Z[k] + conj Z[N-k])/2, B[k] = (Z[k] - conj Z[N-k])/(2i), k = i + TP*t < nkx.
             // Z[k] is this thread's own last-pass output; only Z[N-k] (held by slot (TP-i)%TP) crosses threads.
             // last-pass register m*RL + q holds index i + TP*(m + q*(E/RL)); publish those some k' = N-k can ask for.
+            if constexpr (MHD_XF2_LATEBAR && PL::NP > 1) team_sync<TP>(team);     // the last exchange's reads are done
 #pragma unroll
             for (int m = 0; m < E / RL; ++m)
 #pragma unroll
@@ -257,7 +258,9 @@ __global__ void __launch_bounds__(XCfg2<N>::THREADS, 1) xfused_kernel(XFusedArgs
                         }
                     }
             }
-            team_sync<TP>(team);              // the split reads are done before the next transform's first exchange writes the buffers
+            // the split reads are done before the next transform's first exchange writes the buffers (late-barrier passes
+            // synchronise in front of every write themselves)
+            if constexpr (!(MHD_XF2_LATEBAR && PL::NP > 1)) team_sync<TP>(team);
         }
     }
 }
@@ -362,6 +365,7 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
             }
             XPass2<N, false, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
             // Hermitian split: only Z[N-k] crosses threads (see the fused kernel)
+            if constexpr (MHD_XF2_LATEBAR && PL::NP > 1) team_sync<TP>(team);
 #pragma unroll
             for (int m = 0; m < E / RL; ++m)
 #pragma unroll
@@ -392,7 +396,7 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
                         }
                     }
                 }
-            team_sync<TP>(team);
+            if constexpr (!(MHD_XF2_LATEBAR && PL::NP > 1)) team_sync<TP>(team);
         }
     }
 }

@@ -17,6 +17,16 @@
 #define MHD_XF2_TW 2
 #endif
 
+#ifndef MHD_XF2_LATEBAR
+// XPass2 barrier placement: 0 = write, barrier, read, barrier (the buffers are free again as soon as a pass returns);
+// 1 = barrier, write, barrier, read: the "reads are done" barrier moves in front of the NEXT write, so the reads of an
+// exchange and the twiddle chain / butterflies that consume them are one scheduling region.  Callers then synchronise the
+// team before they write the exchange buffers themselves.  2 = the same, and transform A's writes are issued before
+// transform B's butterflies of the pass, so the load-store pipe drains them under arithmetic.
+// Measured at 512^3 (x_fused, ms): 0: 4.84, 1: 4.76, 2: 4.73 in one session (profiles/r02_experiments.md).
+#define MHD_XF2_LATEBAR 2
+#endif
+
 namespace mhd {
 using namespace mhdfft;
 
@@ -168,8 +178,10 @@ struct XPass2 {
                 }
             }
             bfly<R, INV>(&va[m * R]);
+            if constexpr (MHD_XF2_LATEBAR == 2 && !LAST) continue;     // (the second butterfly and the writes follow below)
             bfly<R, INV>(&vb[m * R]);
             if constexpr (!LAST) {
+                if constexpr (MHD_XF2_LATEBAR) { if (m == 0) team_sync<TP>(team); }     // every reader of the buffers is done
                 if constexpr (P == 1) {            // first pass: j = R*b, element j + q
                     const int j = b * R, pj = xpad(j);
 #pragma unroll
@@ -187,6 +199,34 @@ struct XPass2 {
                 }
             }
         }
+        if constexpr (MHD_XF2_LATEBAR == 2 && !LAST) {
+            // de-bursted order: A's writes are issued, then B's butterflies run while the load-store pipe drains them
+            team_sync<TP>(team);
+#pragma unroll
+            for (int m = 0; m < E / R; ++m) {
+                const int b = i + TP * m, k = b & (P - 1);
+                const int j = (P == 1) ? b * R : (b - k) * R + k, pj = xpad(j);
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    const int o = (P == 1) ? ((R == 8) ? pj + q : xpad(j + q)) : ((P % 8 == 0) ? pj + q * (P + P / 8) : xpad(j + q * P));
+                    smA[o] = va[m * R + q];
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < E; ++e) asm volatile("" : "+d"(vb[e].x), "+d"(vb[e].y));     // keep B's butterflies behind the barrier
+#pragma unroll
+            for (int m = 0; m < E / R; ++m) bfly<R, INV>(&vb[m * R]);
+#pragma unroll
+            for (int m = 0; m < E / R; ++m) {
+                const int b = i + TP * m, k = b & (P - 1);
+                const int j = (P == 1) ? b * R : (b - k) * R + k, pj = xpad(j);
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    const int o = (P == 1) ? ((R == 8) ? pj + q : xpad(j + q)) : ((P % 8 == 0) ? pj + q * (P + P / 8) : xpad(j + q * P));
+                    smB[o] = vb[m * R + q];
+                }
+            }
+        }
         if constexpr (!LAST) {
             constexpr int Rn = PL::radix(S + 1);
             team_sync<TP>(team);
@@ -199,7 +239,7 @@ struct XPass2 {
                     const int o = (D % 8 == 0) ? pi + D + D / 8 : xpad(i + D);
                     va[m * Rn + q] = smA[o]; vb[m * Rn + q] = smB[o];
                 }
-            team_sync<TP>(team);
+            if constexpr (!MHD_XF2_LATEBAR) team_sync<TP>(team);
             XPass2<N, INV, S + 1, P * R>::run(va, vb, smA, smB, i, team, stw);
         }
     }
