@@ -290,6 +290,7 @@ def run_gpu(args):
 
     # ---- measured on-chip ceilings (FP64 FMA pipe, shared-memory data path) for the kernels that are not HBM-bound ----
     fp64_tflops, smem_gbs = mhd.measure_peaks(dev)
+    exch_gbs = mhd.measure_exchange(192, dev)       # the fused pass's exchange pattern alone, with its FP64 work per exchange
 
     # ---- per-kernel rooflines, timed live with CUDA events ----
     abytes = algorithmic_bytes(geo)
@@ -310,6 +311,8 @@ def run_gpu(args):
             floors["smem"] = smem / (smem_gbs * 1e9) * 1e3
             k["fp64_instr"] = dp
             k["smem_bytes"] = smem
+            k["smem_exchange_ceiling_gbs"] = exch_gbs
+            k["frac_of_exchange_ceiling"] = smem / 1e9 / (per * 1e-3) / exch_gbs if exch_gbs > 0 else None
         k["floors_ms"] = floors
         k["bound"] = max(floors, key=floors.get)
         k["frac"] = floors[k["bound"]] / per
@@ -328,10 +331,13 @@ def run_gpu(args):
     roofline = {"bound": top["bound"], "kernel": top["kernel"], "achieved": achieved, "peak": pk, "unit": unit,
                 "frac": top["frac"], "traffic": top["traffic"], "peak_source": what,
                 "hbm_frac": top["hbm_frac"], "hbm_peak": peak, "hbm_peak_source": peak_src,
+                "smem_exchange_ceiling_gbs": top.get("smem_exchange_ceiling_gbs"), "frac_of_exchange_ceiling": top.get("frac_of_exchange_ceiling"),
                 "algorithmic_bytes_per_launch": abytes[top["kernel"]], "floors_ms": top["floors_ms"],
                 "share_of_step": top["share_of_step"],
                 "note": "bound = the highest of the kernel's floors (HBM bytes, FP64 instruction slots, shared-memory bytes; models in "
-                        "DESIGN.md §6); frac = that floor / measured time; hbm_frac is kept beside it"}
+                        "DESIGN.md §6); frac = that floor / measured time; hbm_frac is kept beside it; smem_exchange_ceiling_gbs = what "
+                        "the kernel's own barrier-synchronised exchange pattern reaches with everything else stripped away "
+                        "(mhd_measure_exchange), frac_of_exchange_ceiling = the kernel's shared-memory GB/s over that"}
     own_bytes = sum(k["algorithmic_gb"] * 1e9 * k["launches_per_step"] for k in kernels)   # only the kernel classes that ran
     step_roofline = {
         "design_bytes_per_step": own_bytes, "design_gbs": own_bytes / 1e9 / (ms_step * 1e-3),
@@ -366,7 +372,7 @@ def run_gpu(args):
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
         "peaks": {"hbm_gbs": peak, "hbm_source": peak_src, "fp64_tflops": fp64_tflops, "smem_gbs": smem_gbs,
-                  "onchip_source": "mhd_measure_peaks, this run"},
+                  "smem_exchange_gbs": exch_gbs, "onchip_source": "mhd_measure_peaks / mhd_measure_exchange(192), this run"},
         "fft": fft, "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
@@ -430,6 +436,7 @@ def run_peaks(args):
         raise SystemExit("bench.py: no CUDA device")
     sampler = ClockSampler(0)
     vals = [mhd.measure_peaks("cuda:0") for _ in range(3)]
+    exch = {str(d): max(mhd.measure_exchange(d, "cuda:0") for _ in range(2)) for d in (0, 64, 128, 192, 256)}
     clocks = sampler.stop()
     f, sm = max(v[0] for v in vals), max(v[1] for v in vals)
     sms = torch.cuda.get_device_properties(0).multi_processor_count
@@ -437,6 +444,7 @@ def run_peaks(args):
     line = {"metric": "onchip_peaks", "fp64_tflops": f, "smem_gbs": sm, "clocks": clocks, "sms": sms,
             "dfma_per_clk_per_sm": (f * 1e12 / 2 / sms / (mhz * 1e6)) if mhz else None,
             "smem_bytes_per_clk_per_sm": (sm * 1e9 / sms / (mhz * 1e6)) if mhz else None,
+            "smem_exchange_gbs_by_dfma_per_exchange": exch,
             "hbm_gbs": measured_peak()[0]}
     print(json.dumps(line), flush=True)
     return 0

@@ -1,5 +1,5 @@
 // peaks_kernel.cu — measured ceilings of the two on-chip resources that bound the fused x pass (instrumentation, not on the
-// solver's path): the FP64 FMA pipe and the shared-memory data path.  SURVEY.md §8(d) leaves the FP64 peak "nominal —
+// solver's path): the FP64 FMA pipe and the shared-memory data path, and what the fused pass's own exchange pattern reaches.  SURVEY.md §8(d) leaves the FP64 peak "nominal —
 // builder to measure"; bench.py --workload peaks (and the default bench line) report x_fused against these numbers.
 //
 //   fp64 : every thread runs 8 independent DFMA chains (x = x*a + b), 148*k CTAs of 256 threads, no memory traffic.
@@ -37,6 +37,87 @@ __global__ void __launch_bounds__(256) peak_smem_kernel(double* __restrict__ out
         __syncwarp();
     }
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = v0.x + v1.y + v2.x + v3.y;
+}
+
+// exchange: the fused x pass's own pattern with everything else stripped away.  One persistent CTA of 256 threads per SM,
+//          4 teams of 64 threads; per iteration a thread holds two sets of 8 complex values, runs DFMA_PER_ITER dependent-free
+//          DFMAs on them, and exchanges both sets through team-private padded buffers (barrier, 16 STS.128 with the first-pass
+//          index set, barrier, 16 LDS.128 with the stride-64 index set): what the 8 warps of an SM can pull through the
+//          load-store pipe when the traffic comes in barrier-synchronised bursts with FP64 work in between.
+//          bytes = 32 x 16 per thread per iteration.
+#define MHD_PAD8(e) ((e) + ((e) >> 3))
+template <int REPS>
+__global__ void __launch_bounds__(256, 1) peak_exchange_kernel(double* __restrict__ out, int iters, double a, double b) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    const int team = threadIdx.x / 64, i = threadIdx.x % 64;
+    double2* const A = reinterpret_cast<double2*>(smraw) + (size_t)team * 2 * 640;
+    double2* const B = A + 640;
+    double2 v[8], w[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { v[q] = make_double2(i + q, q); w[q] = make_double2(q, i); }
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < REPS; ++r)
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                v[q].x = fma(v[q].x, a, b); v[q].y = fma(v[q].y, a, -b);
+                w[q].x = fma(w[q].x, a, b); w[q].y = fma(w[q].y, a, -b);
+            }
+        asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { A[MHD_PAD8(i * 8 + q)] = v[q]; B[MHD_PAD8(i * 8 + q)] = w[q]; }
+        asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { v[q] = A[MHD_PAD8(i + 64 * q)]; w[q] = B[MHD_PAD8(i + 64 * q)]; }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += (v[q].x + v[q].y) + (w[q].x + w[q].y);
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// Achieved shared-memory GB/s of the exchange pattern above with 32*REPS DFMAs per thread between exchanges (REPS = 6 is the
+// fused x pass's ratio at N = 512: ~190 FP64 instructions per thread and transform pass).  scratch: >= sms*256 doubles.
+cudaError_t measure_exchange(double* scratch, size_t scratch_doubles, cudaStream_t st, int dfma_per_exchange, double* smem_gbs) {
+    const int dev = device_slot();
+    int sms = 0;
+    cudaError_t e = device_sm_count(dev, &sms);
+    if (e != cudaSuccess) return e;
+    if (scratch_doubles < (size_t)sms * 256) return cudaErrorInvalidValue;
+    const int reps = dfma_per_exchange / 32;
+    void (*kern)(double*, int, double, double) = nullptr;
+    switch (reps) {
+        case 0: kern = peak_exchange_kernel<0>; break;
+        case 2: kern = peak_exchange_kernel<2>; break;
+        case 4: kern = peak_exchange_kernel<4>; break;
+        case 6: kern = peak_exchange_kernel<6>; break;
+        case 8: kern = peak_exchange_kernel<8>; break;
+        default: return cudaErrorInvalidValue;
+    }
+    const int smem = 4 * 2 * 640 * (int)sizeof(double2);
+    if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+    cudaEvent_t a, b;
+    if ((e = cudaEventCreate(&a)) != cudaSuccess) return e;
+    if ((e = cudaEventCreate(&b)) != cudaSuccess) { cudaEventDestroy(a); return e; }
+    double best = 0.0;
+    const int iters = 8192;
+    for (int r = 0; r < 4 && e == cudaSuccess; ++r) {
+        cudaEventRecord(a, st);
+        kern<<<sms, 256, smem, st>>>(scratch, iters, 0.999999, 1e-9);
+        count_launch();
+        cudaEventRecord(b, st);
+        if ((e = cudaEventSynchronize(b)) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        const double bytes = 32.0 * 16.0 * (double)iters * 256.0 * (double)sms;
+        if (r > 0 && ms > 0.f) best = fmax(best, bytes / (ms * 1e-3) / 1e9);
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    *smem_gbs = best;
+    return e;
 }
 
 // scratch: >= grid*256 doubles.  Best of `reps` launches each; results in TFLOP/s and GB/s.

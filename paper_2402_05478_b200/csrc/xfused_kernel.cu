@@ -88,6 +88,8 @@ __global__ void __launch_bounds__(XCfg2<N>::THREADS, 1) xfused_kernel(XFusedArgs
         }
     }
     __syncthreads();
+    cplx wr[4];
+    xpass2_own_twiddles<N>(wr, i, stw);
 
     const long long row_stride = (long long)gridDim.x * CF::TEAMS;
     const unsigned row_bytes = (unsigned)nkx * (unsigned)sizeof(cplx);
@@ -157,7 +159,7 @@ __global__ void __launch_bounds__(XCfg2<N>::THREADS, 1) xfused_kernel(XFusedArgs
                     vb[q] = lo ? make_double2(y0.x - y1.y, y0.y + y1.x) : make_double2(y0.x + y1.y, y1.x - y0.y);
                 }
             }
-            XPass2<N, true, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
+            XPass2<N, true, 0, 1>::run(va, vb, bufA, bufB, i, team, stw, wr);
             if constexpr (PRUNED) {
                 // the staging area of this group is free again: the team has passed a barrier since reading it (a one-thread
                 // team needs none).  Refill it with the same group of the team's next row.
@@ -218,7 +220,7 @@ __global__ void __launch_bounds__(XCfg2<N>::THREADS, 1) xfused_kernel(XFusedArgs
                     break;
             }
             // first-pass input register q must hold x = i + TP*q: that is how va, vb were filled (j = q)
-            XPass2<N, false, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
+            XPass2<N, false, 0, 1>::run(va, vb, bufA, bufB, i, team, stw, wr);
             // Hermitian split: A[k] = (Z[k] + conj Z[N-k])/2, B[k] = (Z[k] - conj Z[N-k])/(2i), k = i + TP*t < nkx.
             // Z[k] is this thread's own last-pass output; only Z[N-k] (held by slot (TP-i)%TP) crosses threads.
             // last-pass register m*RL + q holds index i + TP*(m + q*(E/RL)); publish those some k' = N-k can ask for.
@@ -304,6 +306,8 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
         }
     }
     __syncthreads();
+    cplx wr[4];
+    xpass2_own_twiddles<N>(wr, i, stw);
     // a team takes TWO row pairs per iteration (two transforms in flight per thread, XPass2): the kernel is latency-bound
     const long long npairs = (a.nrows + 1) / 2;
     const long long nunits = (npairs + 1) / 2;
@@ -347,7 +351,7 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
                 va[q] = lo ? make_double2(x0.x - x1.y, x0.y + x1.x) : make_double2(x0.x + x1.y, x1.x - x0.y);
                 vb[q] = lo ? make_double2(y0.x - y1.y, y0.y + y1.x) : make_double2(y0.x + y1.y, y1.x - y0.y);
             }
-            XPass2<N, true, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
+            XPass2<N, true, 0, 1>::run(va, vb, bufA, bufB, i, team, stw, wr);
             const double s = a.scale;
 #pragma unroll
             for (int m = 0; m < E / RL; ++m)
@@ -363,7 +367,7 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
                 va[q] = oka ? make_double2(ra0[i + TP * q], ra1[i + TP * q]) : make_double2(0.0, 0.0);
                 vb[q] = okb ? make_double2(rb0[i + TP * q], rb1[i + TP * q]) : make_double2(0.0, 0.0);
             }
-            XPass2<N, false, 0, 1>::run(va, vb, bufA, bufB, i, team, stw);
+            XPass2<N, false, 0, 1>::run(va, vb, bufA, bufB, i, team, stw, wr);
             // Hermitian split: only Z[N-k] crosses threads (see the fused kernel)
             if constexpr (MHD_XF2_LATEBAR && PL::NP > 1) team_sync<TP>(team);
 #pragma unroll

@@ -17,6 +17,11 @@
 #define MHD_XF2_TW 2
 #endif
 
+#ifndef MHD_XF2_TWREG
+// 1: the thread's own w of every radix-8 pass lives in registers for the whole kernel (4 doubles at N = 512) instead of
+// being re-read from the shared table by every transform pair
+#define MHD_XF2_TWREG 1
+#endif
 #ifndef MHD_XF2_LATEBAR
 // XPass2 barrier placement: 0 = write, barrier, read, barrier (the buffers are free again as soon as a pass returns);
 // 1 = barrier, write, barrier, read: the "reads are done" barrier moves in front of the NEXT write, so the reads of an
@@ -131,6 +136,22 @@ struct XPass {
 };
 
 
+// the thread's twiddles w of the radix-8 passes S >= 1 (8 points per thread: one butterfly per pass, k = i mod P): they do not
+// depend on the row, so the x kernels read them from the shared tables once, before their row loop
+template <int N> __device__ __forceinline__ void xpass2_own_twiddles(cplx (&wr)[4], int i, const cplx* __restrict__ stw) {
+    using PL = Plan<N>;
+    int P = PL::radix(0);
+#pragma unroll
+    for (int s = 1; s < 4; ++s) {
+        wr[s] = make_double2(1.0, 0.0);
+        if (s < PL::NP) {
+            if (PL::radix(s) == 8) wr[s] = stw[XCfg<N>::tw_offset(s) + (i & (P - 1))];
+            P *= PL::radix(s);
+        }
+    }
+    wr[0] = make_double2(1.0, 0.0);
+}
+
 // Two independent transforms per thread (va, vb), pass by pass in lock step: the twiddles of a pass are formed once and
 // applied to both, one team barrier serves both exchanges, and the two butterflies give every warp two independent
 // instruction streams (the fused x pass is latency-bound: 12 warps per SM cannot cover the FP64 and shared-memory
@@ -142,7 +163,9 @@ struct XPass2 {
     static constexpr int E = PL::E;
     static constexpr int TP = PL::TP;
     static constexpr bool LAST = (S == PL::NP - 1);
-    __device__ __forceinline__ static void run(cplx (&va)[E], cplx (&vb)[E], cplx* smA, cplx* smB, int i, int team, const cplx* __restrict__ stw) {
+    // wr[S]: the thread's own twiddle w of a radix-8 pass S (it depends on the slot i only), kept in registers by the caller
+    __device__ __forceinline__ static void run(cplx (&va)[E], cplx (&vb)[E], cplx* smA, cplx* smB, int i, int team, const cplx* __restrict__ stw,
+                                               const cplx (&wr)[4]) {
 #pragma unroll
         for (int m = 0; m < E / R; ++m) {
             const int b = i + TP * m;
@@ -150,7 +173,7 @@ struct XPass2 {
             if constexpr (S > 0) {
                 const cplx* __restrict__ t = stw + XCfg<N>::tw_offset(S) + k;
                 if constexpr (R == 8 && (MHD_XF2_TW == 2 || (MHD_XF2_TW == 3 && P >= 32) || (MHD_XF2_TW == 1 && P >= 32))) {
-                    cplx w1 = t[0], w2, w3, w4, w5, w6, w7;
+                    cplx w1 = (MHD_XF2_TWREG && E == 8) ? wr[S] : t[0], w2, w3, w4, w5, w6, w7;
                     if (INV) w1.y = -w1.y;
                     if constexpr (MHD_XF2_TW == 3) {      // w, w^2, w^4 from the table, four products of depth 1
                         w2 = t[P]; w4 = t[3 * P];
@@ -240,7 +263,7 @@ struct XPass2 {
                     va[m * Rn + q] = smA[o]; vb[m * Rn + q] = smB[o];
                 }
             if constexpr (!MHD_XF2_LATEBAR) team_sync<TP>(team);
-            XPass2<N, INV, S + 1, P * R>::run(va, vb, smA, smB, i, team, stw);
+            XPass2<N, INV, S + 1, P * R>::run(va, vb, smA, smB, i, team, stw, wr);
         }
     }
 };

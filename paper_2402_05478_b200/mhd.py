@@ -26,7 +26,7 @@ EXPORTS = [
     "mhd_get_fields", "mhd_get_fields_host", "mhd_diagnostics", "mhd_strerror", "mhd_last_error",
     "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy", "mhd_fft_last_error", "mhd_fft_plan_set_mode",
     "mhd_launch_count", "mhd_profile_kernel_count", "mhd_profile_kernel_name", "mhd_profile_begin", "mhd_profile_end",
-    "mhd_measure_peaks",
+    "mhd_measure_peaks", "mhd_measure_exchange",
 ]
 
 
@@ -94,6 +94,7 @@ def lib():
         L.mhd_profile_begin.argtypes = [_vp]
         L.mhd_profile_end.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.mhd_measure_peaks.argtypes = [_vp, C.c_size_t, _vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.mhd_measure_exchange.argtypes = [_vp, C.c_size_t, _vp, C.c_int, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -115,6 +116,21 @@ def measure_peaks(device="cuda:0"):
     if rc != OK:
         raise MhdError(rc, "mhd_measure_peaks")
     return float(f.value), float(s.value)
+
+
+def measure_exchange(dfma_per_exchange=192, device="cuda:0"):
+    """shared-memory GB/s reached by the fused x pass's exchange pattern alone (mhd_measure_exchange)."""
+    torch = _torch()
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        scratch = torch.empty(8 << 20, dtype=torch.uint8, device=dev)
+        g = C.c_double()
+        torch.cuda.synchronize(dev)
+        rc = lib().mhd_measure_exchange(_vp(scratch.data_ptr()), scratch.numel(), _vp(torch.cuda.current_stream(dev).cuda_stream),
+                                        int(dfma_per_exchange), C.byref(g))
+    if rc != OK:
+        raise MhdError(rc, "mhd_measure_exchange")
+    return float(g.value)
 
 
 def _torch():
