@@ -437,6 +437,8 @@ def run_peaks(args):
     sampler = ClockSampler(0)
     vals = [mhd.measure_peaks("cuda:0") for _ in range(3)]
     exch = {str(d): max(mhd.measure_exchange(d, "cuda:0") for _ in range(2)) for d in (0, 64, 128, 192, 256)}
+    exch_modes = {name: max(mhd.measure_exchange(192, "cuda:0", m) for _ in range(2))
+                  for m, name in enumerate(("write_barrier_read_barrier", "barrier_write_barrier_read", "double_buffer_one_barrier"))}
     clocks = sampler.stop()
     f, sm = max(v[0] for v in vals), max(v[1] for v in vals)
     sms = torch.cuda.get_device_properties(0).multi_processor_count
@@ -444,7 +446,7 @@ def run_peaks(args):
     line = {"metric": "onchip_peaks", "fp64_tflops": f, "smem_gbs": sm, "clocks": clocks, "sms": sms,
             "dfma_per_clk_per_sm": (f * 1e12 / 2 / sms / (mhz * 1e6)) if mhz else None,
             "smem_bytes_per_clk_per_sm": (sm * 1e9 / sms / (mhz * 1e6)) if mhz else None,
-            "smem_exchange_gbs_by_dfma_per_exchange": exch,
+            "smem_exchange_gbs_by_dfma_per_exchange": exch, "smem_exchange_gbs_by_barrier_placement_at_192": exch_modes,
             "hbm_gbs": measured_peak()[0]}
     print(json.dumps(line), flush=True)
     return 0

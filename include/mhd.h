@@ -182,11 +182,14 @@ int mhd_profile_end(mhd_ctx* ctx, int* counts_host, double* ms_host);
 int mhd_measure_peaks(void* scratch_dev, size_t scratch_bytes, void* cuda_stream, double* fp64_tflops_host, double* smem_gbs_host);
 
 /* What the fused x pass's own shared-memory exchange pattern reaches with everything else stripped away: 4 teams of 64 threads
- * per SM, per iteration dfma_per_exchange (0, 64, 128, 192 or 256) independent DFMAs per thread, a team barrier, 16 STS.128, a
- * team barrier, 16 LDS.128 (the padded index sets of the Stockham passes).  Result: GB/s moved through shared memory.  The
- * fused pass at N = 512 has ~190 FP64 instructions per thread between exchanges; its achievable ceiling is this number, not the
- * free-running shared-memory peak of mhd_measure_peaks.  scratch_dev as above; synchronises; MHD_EINVAL for other counts. */
-int mhd_measure_exchange(void* scratch_dev, size_t scratch_bytes, void* cuda_stream, int dfma_per_exchange, double* smem_gbs_host);
+ * per SM, per iteration dfma_per_exchange (0, 64, 128, 192 or 256) independent DFMAs per thread, then 16 STS.128 and 16 LDS.128
+ * (the padded index sets of the Stockham passes) with team barriers placed by barrier_mode: 0 = write, barrier, read, barrier;
+ * 1 = barrier, write, barrier, read (the shipped x passes); 2 = two buffers used alternately, one barrier per exchange.
+ * Result: GB/s moved through shared memory.  The fused pass at N = 512 has ~190 FP64 instructions per thread between
+ * exchanges; its achievable ceiling is this number, not the free-running shared-memory peak of mhd_measure_peaks.
+ * scratch_dev as above; synchronises; MHD_EINVAL for other counts or modes. */
+int mhd_measure_exchange(void* scratch_dev, size_t scratch_bytes, void* cuda_stream, int dfma_per_exchange, int barrier_mode,
+                         double* smem_gbs_host);
 
 #ifdef __cplusplus
 }

@@ -306,11 +306,12 @@ int mhd_measure_peaks(void* scratch, size_t bytes, void* stream, double* fp64_tf
     return measure_peaks((double*)scratch, bytes / sizeof(double), (cudaStream_t)stream, fp64_tflops, smem_gbs) == cudaSuccess ? MHD_OK : MHD_ECUDA;
 }
 
-int mhd_measure_exchange(void* scratch, size_t bytes, void* stream, int dfma_per_exchange, double* smem_gbs) {
+int mhd_measure_exchange(void* scratch, size_t bytes, void* stream, int dfma_per_exchange, int barrier_mode, double* smem_gbs) {
     if (!scratch || !smem_gbs || bytes < ((size_t)4 << 20)) return MHD_EINVAL;
     if (dfma_per_exchange < 0 || dfma_per_exchange > 256 || dfma_per_exchange % 64 != 0) return MHD_EINVAL;
+    if (barrier_mode < 0 || barrier_mode > 2) return MHD_EINVAL;
     DeviceGuard guard(owning_device(scratch));
-    return measure_exchange((double*)scratch, bytes / sizeof(double), (cudaStream_t)stream, dfma_per_exchange, smem_gbs) == cudaSuccess ? MHD_OK : MHD_ECUDA;
+    return measure_exchange((double*)scratch, bytes / sizeof(double), (cudaStream_t)stream, dfma_per_exchange, barrier_mode, smem_gbs) == cudaSuccess ? MHD_OK : MHD_ECUDA;
 }
 
 int mhd_profile_begin(mhd_ctx* c) {

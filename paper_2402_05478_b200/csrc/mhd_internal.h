@@ -114,7 +114,8 @@ void add_launches(long long n);
 cudaError_t measure_peaks(double* scratch, size_t scratch_doubles, cudaStream_t st, double* fp64_tflops, double* smem_gbs);
 // shared-memory GB/s of the fused x pass's exchange pattern (team barriers, bursts of 16 + 16 accesses) with dfma_per_exchange
 // (0, 64, ..., 256) DFMAs per thread in between
-cudaError_t measure_exchange(double* scratch, size_t scratch_doubles, cudaStream_t st, int dfma_per_exchange, double* smem_gbs);
+// mode: 0 write-barrier-read-barrier, 1 barrier-write-barrier-read (shipped), 2 double-buffered, one barrier per exchange
+cudaError_t measure_exchange(double* scratch, size_t scratch_doubles, cudaStream_t st, int dfma_per_exchange, int mode, double* smem_gbs);
 
 // ---- per-device one-time kernel setup ---------------------------------------------------------------
 // cudaFuncSetAttribute (opt-in dynamic shared memory) and the SM count belong to a DEVICE, not to the process: every

@@ -42,16 +42,17 @@ __global__ void __launch_bounds__(256) peak_smem_kernel(double* __restrict__ out
 // exchange: the fused x pass's own pattern with everything else stripped away.  One persistent CTA of 256 threads per SM,
 //          4 teams of 64 threads; per iteration a thread holds two sets of 8 complex values, runs DFMA_PER_ITER dependent-free
 //          DFMAs on them, and exchanges both sets through team-private padded buffers (barrier, 16 STS.128 with the first-pass
-//          index set, barrier, 16 LDS.128 with the stride-64 index set): what the 8 warps of an SM can pull through the
+//          index set, barrier, 16 LDS.128 with the stride-64 index set; see MODE): what the 8 warps of an SM can pull through the
 //          load-store pipe when the traffic comes in barrier-synchronised bursts with FP64 work in between.
 //          bytes = 32 x 16 per thread per iteration.
 #define MHD_PAD8(e) ((e) + ((e) >> 3))
-template <int REPS>
+// MODE 0: write, barrier, read, barrier; 1: barrier, write, barrier, read (the shipped x passes); 2: two buffers per set used
+// alternately, ONE barrier per exchange (write, barrier, read)
+template <int REPS, int MODE>
 __global__ void __launch_bounds__(256, 1) peak_exchange_kernel(double* __restrict__ out, int iters, double a, double b) {
     extern __shared__ __align__(16) unsigned char smraw[];
     const int team = threadIdx.x / 64, i = threadIdx.x % 64;
-    double2* const A = reinterpret_cast<double2*>(smraw) + (size_t)team * 2 * 640;
-    double2* const B = A + 640;
+    double2* const base = reinterpret_cast<double2*>(smraw) + (size_t)team * 4 * 640;
     double2 v[8], w[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) { v[q] = make_double2(i + q, q); w[q] = make_double2(q, i); }
@@ -64,12 +65,15 @@ __global__ void __launch_bounds__(256, 1) peak_exchange_kernel(double* __restric
                 v[q].x = fma(v[q].x, a, b); v[q].y = fma(v[q].y, a, -b);
                 w[q].x = fma(w[q].x, a, b); w[q].y = fma(w[q].y, a, -b);
             }
-        asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
+        double2* const A = base + ((MODE == 2) ? (it & 1) * 1280 : 0);
+        double2* const B = A + 640;
+        if (MODE == 1) asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
 #pragma unroll
         for (int q = 0; q < 8; ++q) { A[MHD_PAD8(i * 8 + q)] = v[q]; B[MHD_PAD8(i * 8 + q)] = w[q]; }
         asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
 #pragma unroll
         for (int q = 0; q < 8; ++q) { v[q] = A[MHD_PAD8(i + 64 * q)]; w[q] = B[MHD_PAD8(i + 64 * q)]; }
+        if (MODE == 0) asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
     }
     double s = 0.0;
 #pragma unroll
@@ -79,7 +83,7 @@ __global__ void __launch_bounds__(256, 1) peak_exchange_kernel(double* __restric
 
 // Achieved shared-memory GB/s of the exchange pattern above with 32*REPS DFMAs per thread between exchanges (REPS = 6 is the
 // fused x pass's ratio at N = 512: ~190 FP64 instructions per thread and transform pass).  scratch: >= sms*256 doubles.
-cudaError_t measure_exchange(double* scratch, size_t scratch_doubles, cudaStream_t st, int dfma_per_exchange, double* smem_gbs) {
+cudaError_t measure_exchange(double* scratch, size_t scratch_doubles, cudaStream_t st, int dfma_per_exchange, int mode, double* smem_gbs) {
     const int dev = device_slot();
     int sms = 0;
     cudaError_t e = device_sm_count(dev, &sms);
@@ -87,15 +91,15 @@ cudaError_t measure_exchange(double* scratch, size_t scratch_doubles, cudaStream
     if (scratch_doubles < (size_t)sms * 256) return cudaErrorInvalidValue;
     const int reps = dfma_per_exchange / 32;
     void (*kern)(double*, int, double, double) = nullptr;
+#define MHD_EXCH(R_)                                                                              \
+    case R_: kern = mode == 0 ? peak_exchange_kernel<R_, 0> : mode == 1 ? peak_exchange_kernel<R_, 1> : peak_exchange_kernel<R_, 2>; break;
+    if (mode < 0 || mode > 2) return cudaErrorInvalidValue;
     switch (reps) {
-        case 0: kern = peak_exchange_kernel<0>; break;
-        case 2: kern = peak_exchange_kernel<2>; break;
-        case 4: kern = peak_exchange_kernel<4>; break;
-        case 6: kern = peak_exchange_kernel<6>; break;
-        case 8: kern = peak_exchange_kernel<8>; break;
+        MHD_EXCH(0) MHD_EXCH(2) MHD_EXCH(4) MHD_EXCH(6) MHD_EXCH(8)
         default: return cudaErrorInvalidValue;
     }
-    const int smem = 4 * 2 * 640 * (int)sizeof(double2);
+#undef MHD_EXCH
+    const int smem = 4 * 4 * 640 * (int)sizeof(double2);
     if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
     cudaEvent_t a, b;
     if ((e = cudaEventCreate(&a)) != cudaSuccess) return e;

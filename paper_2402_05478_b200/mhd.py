@@ -94,7 +94,7 @@ def lib():
         L.mhd_profile_begin.argtypes = [_vp]
         L.mhd_profile_end.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.mhd_measure_peaks.argtypes = [_vp, C.c_size_t, _vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
-        L.mhd_measure_exchange.argtypes = [_vp, C.c_size_t, _vp, C.c_int, C.POINTER(C.c_double)]
+        L.mhd_measure_exchange.argtypes = [_vp, C.c_size_t, _vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -118,7 +118,7 @@ def measure_peaks(device="cuda:0"):
     return float(f.value), float(s.value)
 
 
-def measure_exchange(dfma_per_exchange=192, device="cuda:0"):
+def measure_exchange(dfma_per_exchange=192, device="cuda:0", barrier_mode=1):
     """shared-memory GB/s reached by the fused x pass's exchange pattern alone (mhd_measure_exchange)."""
     torch = _torch()
     dev = torch.device(device)
@@ -127,7 +127,7 @@ def measure_exchange(dfma_per_exchange=192, device="cuda:0"):
         g = C.c_double()
         torch.cuda.synchronize(dev)
         rc = lib().mhd_measure_exchange(_vp(scratch.data_ptr()), scratch.numel(), _vp(torch.cuda.current_stream(dev).cuda_stream),
-                                        int(dfma_per_exchange), C.byref(g))
+                                        int(dfma_per_exchange), int(barrier_mode), C.byref(g))
     if rc != OK:
         raise MhdError(rc, "mhd_measure_exchange")
     return float(g.value)

@@ -116,9 +116,10 @@ def test_peaks_probe_rejects_bad_arguments(lib):
     f, s = C.c_double(), C.c_double()
     assert lib.mhd_measure_peaks(None, 1 << 23, None, C.byref(f), C.byref(s)) == mhd.EINVAL
     assert lib.mhd_measure_peaks(C.c_void_p(256), 16, None, C.byref(f), C.byref(s)) == mhd.EINVAL
-    assert lib.mhd_measure_exchange(None, 1 << 23, None, 192, C.byref(s)) == mhd.EINVAL
-    assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 100, C.byref(s)) == mhd.EINVAL     # not a multiple of 64
-    assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 320, C.byref(s)) == mhd.EINVAL
+    assert lib.mhd_measure_exchange(None, 1 << 23, None, 192, 1, C.byref(s)) == mhd.EINVAL
+    assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 100, 1, C.byref(s)) == mhd.EINVAL     # not a multiple of 64
+    assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 320, 1, C.byref(s)) == mhd.EINVAL
+    assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 192, 3, C.byref(s)) == mhd.EINVAL     # no such barrier mode
     assert lib.mhd_fft_last_error(None) == b""
     assert lib.mhd_fft_plan_set_mode(None, 0) == mhd.EINVAL
     # the plane pipeline needs a ring + counters in the plan workspace only for square planes of 64..512
