@@ -27,8 +27,11 @@ __device__ __forceinline__ int compact_index(int f, int n, int nk) {
     return -1;
 }
 
+#ifndef MHD_AXIS24_MINB
+#define MHD_AXIS24_MINB 2     // minimum CTAs per SM asked of ptxas for the 24-points-per-thread lengths (0: no request)
+#endif
 template <int N, bool INV>
-__global__ void __launch_bounds__(Tile<N>::THREADS) fft_axis_kernel(AxisArgs a, const cplx* __restrict__ tw) {
+__global__ void __launch_bounds__(Tile<N>::THREADS, (Plan<N>::E == 24 ? MHD_AXIS24_MINB : 0)) fft_axis_kernel(AxisArgs a, const cplx* __restrict__ tw) {
     extern __shared__ __align__(16) unsigned char smraw[];
     using PL = Plan<N>;
     const int tid = threadIdx.x, p = tid & 7, i = (tid >> 3) % PL::TP, g = tid / (8 * PL::TP);

@@ -117,8 +117,14 @@ __device__ __forceinline__ double wavenum(int j, int nk) { return (double)((j < 
 
 __device__ __forceinline__ double2 axpy(double2 a, double s, double2 r) { return make_double2(a.x + s * r.x, a.y + s * r.y); }
 
-template <bool HYDRO>
+#ifndef MHD_STAGE_SPLIT
+#define MHD_STAGE_SPLIT 1      // 1: the MHD stage runs as two launches, (rho, m) then B: fewer concurrent streams per kernel
+#endif
+// PART 0: all seven fields; 1: rho and m only (the whole stage of a hydrodynamic run); 2: B only
+template <int PART>
 __global__ void __launch_bounds__(kThreads) stage_kernel(StageArgs a) {
+    constexpr bool HYDRO = (PART == 1);
+    constexpr int F0 = (PART == 2) ? F_BX : 0, F1 = (PART == 1) ? 4 : NFIELD;
     const SpecGeom g = a.g;
     const long long total = g.field;
     const long long F = g.field;
@@ -132,16 +138,16 @@ __global__ void __launch_bounds__(kThreads) stage_kernel(StageArgs a) {
 
         double2 S[NFIELD], R[NFIELD];
 #pragma unroll
-        for (int f = 0; f < (HYDRO ? 4 : NFIELD); ++f) S[f] = a.S[f * F + idx];
+        for (int f = F0; f < F1; ++f) S[f] = a.S[f * F + idx];
         const double2* __restrict__ G = a.G + idx;
         // eq. (1): R_rho = -i k.m^
-        {
+        if (PART != 2) {
             const double dx = kx * S[F_MX].x + ky * S[F_MY].x + kz * S[F_MZ].x;
             const double dy = kx * S[F_MX].y + ky * S[F_MY].y + kz * S[F_MZ].y;
             R[F_RHO] = make_double2(dy, -dx);
         }
         // eqs (2)+(3): R_m,i = -i k_j T^_ij - i k_i cs^2 rho^ - nu k^2 u^_i
-        {
+        if (PART != 2) {
             const double2 txx = G[P_TXX * F], tyy = G[P_TYY * F], tzz = G[P_TZZ * F];
             const double2 txy = G[P_TXY * F], txz = G[P_TXZ * F], tyz = G[P_TYZ * F];
             const double2 ux = G[P_UX * F], uy = G[P_UY * F], uz = G[P_UZ * F];
@@ -173,7 +179,7 @@ __global__ void __launch_bounds__(kThreads) stage_kernel(StageArgs a) {
         }
         const double dt = a.dt;
 #pragma unroll
-        for (int f = 0; f < (HYDRO ? 4 : NFIELD); ++f) {
+        for (int f = F0; f < F1; ++f) {
             const long long o = f * F + idx;
             switch (a.mode) {
                 case STAGE_AB2_EULER: a.S[o] = axpy(S[f], dt, R[f]); a.H[o] = R[f]; break;
@@ -194,8 +200,12 @@ __global__ void __launch_bounds__(kThreads) stage_kernel(StageArgs a) {
 cudaError_t launch_stage(const StageArgs& a, cudaStream_t st) {
     long long blocks = (a.g.field + kThreads - 1) / kThreads;
     if (blocks > kGridStream) blocks = kGridStream;
-    if (a.hydro) stage_kernel<true><<<(unsigned)blocks, kThreads, 0, st>>>(a);
-    else stage_kernel<false><<<(unsigned)blocks, kThreads, 0, st>>>(a);
+    if (a.hydro) stage_kernel<1><<<(unsigned)blocks, kThreads, 0, st>>>(a);
+    else if (MHD_STAGE_SPLIT) {
+        stage_kernel<1><<<(unsigned)blocks, kThreads, 0, st>>>(a);
+        count_launch();
+        stage_kernel<2><<<(unsigned)blocks, kThreads, 0, st>>>(a);
+    } else stage_kernel<0><<<(unsigned)blocks, kThreads, 0, st>>>(a);
     count_launch();
     return cudaGetLastError();
 }
