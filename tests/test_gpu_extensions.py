@@ -232,3 +232,19 @@ def test_exact_resume_is_bit_identical(gpu, integrator):
     with pytest.raises(gpu.MhdError) as e:
         other.get_state()
     assert e.value.code == gpu.ESTATE
+
+
+def test_onchip_probes_are_consistent(gpu):
+    """Instrumentation (bench.py's on-chip ceilings): the FP64 and shared-memory probes land near the hardware's nominal rates,
+    and the fused pass's exchange pattern can never beat the free-running shared-memory probe."""
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    fp64, smem = gpu.measure_peaks("cuda:0")
+    assert 10.0 < fp64 < 2.0 * 64 * sms * 2.2e9 / 1e12              # TFLOP/s: positive, below 64 DFMA/clk/SM at 2.2 GHz
+    assert 5e3 < smem < 128.0 * sms * 2.2                            # GB/s: below 128 B/clk/SM at 2.2 GHz
+    for mode in (0, 1, 2):
+        ex = gpu.measure_exchange(192, "cuda:0", mode)
+        assert 0.5 * smem < ex < 1.02 * smem, (mode, ex, smem)
+    assert gpu.measure_exchange(0, "cuda:0") >= 0.95 * gpu.measure_exchange(256, "cuda:0")     # FP64 work never speeds the exchange up
+    with pytest.raises(gpu.MhdError):
+        gpu.measure_exchange(100, "cuda:0")
