@@ -168,7 +168,8 @@ long long mhd_launch_count(void);
  * eagerly with a CUDA-event pair around every launch (on the context's stream); mhd_profile_end
  * synchronises, fills counts[i] (launches) and ms[i] (summed device time) for the
  * mhd_profile_kernel_count() kernel classes named by mhd_profile_kernel_name(i) -- in hot-path
- * order: z inverse, y inverse, x C2R, products, x R2C, fused x pass, y forward, z forward, stage -- and switches
+ * order: z inverse, y inverse, x C2R, products, x R2C, fused x pass, y forward, z forward, stage (its two launches, (rho, m)
+ * and B, counted as one) -- and switches
  * profiling off.  Both arrays are HOST memory of that length. */
 int mhd_profile_kernel_count(void);
 const char* mhd_profile_kernel_name(int i);
