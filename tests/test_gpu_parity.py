@@ -146,8 +146,16 @@ def test_hydro_flag_keeps_B_exactly_zero_and_matches_unflagged_run(gpu, ref):
     g2 = gpu.Solver(32, 32, 32, 0.02, 0.0, 1.0, 2e-3)
     g2.set_fields(*[torch.from_numpy(a).cuda() for a in f])
     g2.step(cfg.steps)
-    for a, b in zip(got[:4], g2.get_fields()[:4]):
+    got2 = g2.get_fields()
+    for a, b in zip(got[:4], got2[:4]):
         assert torch.equal(a, b)
+    # ... and B = 0 is an invariant of eq. (4): the unflagged run must keep it EXACTLY (no roundoff leak of T_yz into E_x through
+    # the shared transform of the pair: the x transform of a real row is Hermitian to the bit); the oracle does (DESIGN.md §2 #14)
+    assert all(not bool(t.any()) for t in got2[4:])
+    o2 = ref.RefSolver(32, 32, 32, 0.02, 0.0, 1.0, 2e-3)            # the unflagged oracle on the same state
+    o2.set_fields(*f)
+    o2.step(cfg.steps)
+    assert all(not np.any(a) for a in o2.get_fields()[4:])
     # hydro set_fields accepts missing B
     g3 = gpu.Solver(32, 32, 32, 0.02, 0.0, 1.0, 2e-3, flags=1)
     g3.set_fields(*[torch.from_numpy(a).cuda() for a in f[:4]])
