@@ -405,6 +405,117 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
     }
 }
 
+// Inverse x rows with TMA-staged inputs (N >= 256, 8 points per thread): the plain inverse kernel above spends its time waiting
+// for its row loads (ncu: long scoreboard, 56 % of the DRAM rate against 78 % for the forward direction).  Here one persistent
+// CTA per SM runs the fused pass's scheme: a team's NEXT unit (four consecutive half-spectrum rows = one contiguous block) is
+// brought into shared memory by one bulk copy (cp.async.bulk + mbarrier, two staging buffers per team) while the current unit
+// is transformed, so no warp ever waits on a global load.
+#ifndef MHD_XROWS_INV_STAGED
+#define MHD_XROWS_INV_STAGED 1
+#endif
+template <int N> struct XRowStagedCfg {
+    static constexpr int TP = Plan<N>::TP;
+    static constexpr int THREADS = 256;
+    static constexpr int TEAMS = THREADS / TP;
+    static constexpr int NTW = XCfg<N>::NTW > 0 ? XCfg<N>::NTW : 1;
+    __host__ __device__ static size_t smem(long long pitch) {       // exchange buffers, twiddle tables, 2 x 4 staged rows per team, mbarriers
+        return sizeof(cplx) * ((size_t)2 * XCfg<N>::BUF * TEAMS + NTW + (size_t)TEAMS * 8 * pitch) + 16 * (size_t)TEAMS;
+    }
+};
+
+template <int N>
+__global__ void __launch_bounds__(XRowStagedCfg<N>::THREADS, 1) xrows_inv_staged_kernel(RowArgs a, const cplx* __restrict__ tw) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    using PL = Plan<N>;
+    using CF = XCfg<N>;
+    using RC = XRowStagedCfg<N>;
+    static_assert(PL::E == 8 && RC::TEAMS >= 1, "staged inverse x rows: 8 points per thread");
+    constexpr int TP = PL::TP, E = 8;
+    constexpr int RL = PL::radix(PL::NP - 1);
+    const int team = threadIdx.x / TP, i = threadIdx.x % TP;
+    cplx* const smbase = reinterpret_cast<cplx*>(smraw);
+    cplx* const stw = smbase + (size_t)2 * CF::BUF * RC::TEAMS;
+    cplx* const bufA = smbase + (size_t)team * 2 * CF::BUF;
+    cplx* const bufB = bufA + CF::BUF;
+    const int nkx = a.nkx;
+    const long long pitch = a.spec_pitch;
+    cplx* const stage = stw + RC::NTW + (size_t)team * 8 * pitch;                  // two buffers of 4 rows
+    unsigned long long* const mbar = reinterpret_cast<unsigned long long*>(stw + RC::NTW + (size_t)RC::TEAMS * 8 * pitch) + 2 * team;
+    if (i == 0) { mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    {
+        int P = PL::radix(0);
+#pragma unroll
+        for (int s = 1; s < PL::NP; ++s) {
+            const int R = PL::radix(s), off = CF::tw_offset(s);
+            for (int e = threadIdx.x; e < (R - 1) * P; e += blockDim.x) {
+                const int q = e / P + 1, k = e % P;
+                stw[off + e] = tw[k * q * (N / (P * R))];
+            }
+            P *= R;
+        }
+    }
+    __syncthreads();
+    cplx wr[4];
+    xpass2_own_twiddles<N>(wr, i, stw);
+
+    const long long npairs = (a.nrows + 1) / 2;
+    const long long nunits = (npairs + 1) / 2;
+    const long long stride = (long long)gridDim.x * RC::TEAMS;
+    // rows 4u .. 4u+3 of unit u are one contiguous block of the spectrum array (fewer at the end of the batch)
+    auto stage_unit = [&](long long u, int b) {
+        const long long left = a.nrows - 4 * u;
+        const unsigned bytes = (unsigned)((left < 4 ? left : 4) * pitch * (long long)sizeof(cplx));
+        mbar_expect_tx(&mbar[b], bytes);
+        bulk_g2s(stage + (size_t)b * 4 * pitch, a.spec + 4 * u * pitch, bytes, &mbar[b]);
+    };
+    const long long u0 = (long long)blockIdx.x * RC::TEAMS + team;
+    if (i == 0 && u0 < nunits) stage_unit(u0, 0);
+    unsigned phase = 0;          // bit b = parity the next wait on mbar[b] expects
+    int b = 0;
+    for (long long u = u0; u - team < nunits; u += stride, b ^= 1) {
+        const bool oku = u < nunits;
+        const bool oka = oku && 2 * u < npairs, okb = oku && 2 * u + 1 < npairs;
+        // every thread of the team has finished reading buffer b^1 (it passed the team barriers of the previous transform)
+        if (i == 0 && u + stride < nunits) stage_unit(u + stride, b ^ 1);
+        if (oku) { mbar_wait(&mbar[b], (phase >> b) & 1u); phase ^= 1u << b; }
+        const cplx* __restrict__ A0 = stage + (size_t)b * 4 * pitch;
+        const cplx* __restrict__ A1 = A0 + pitch;
+        const cplx* __restrict__ B0 = A1 + pitch;
+        const cplx* __restrict__ B1 = B0 + pitch;
+        const long long r0 = oka ? 4 * u : 0, r1 = okb ? 4 * u + 2 : 0;
+        double* __restrict__ ra0 = a.real + r0 * a.real_pitch;
+        double* __restrict__ ra1 = ra0 + a.real_pitch;
+        double* __restrict__ rb0 = a.real + r1 * a.real_pitch;
+        double* __restrict__ rb1 = rb0 + a.real_pitch;
+        cplx va[E], vb[E];
+#pragma unroll
+        for (int q = 0; q < E; ++q) {                 // first-pass input k = i + TP*q
+            const int k = i + TP * q;
+            const bool lo = k < nkx, hi = (N - k) < nkx;
+            const int idx = lo ? k : N - k;
+            cplx x0 = make_double2(0.0, 0.0), x1 = x0, y0 = x0, y1 = x0;
+            if (lo || hi) {
+                if (oka) { x0 = A0[idx]; x1 = A1[idx]; }
+                if (okb) { y0 = B0[idx]; y1 = B1[idx]; }
+            }
+            if (k == 0 || 2 * k == N) { x0.y = 0.0; x1.y = 0.0; y0.y = 0.0; y1.y = 0.0; }   // self-conjugate modes: Im ignored
+            va[q] = lo ? make_double2(x0.x - x1.y, x0.y + x1.x) : make_double2(x0.x + x1.y, x1.x - x0.y);
+            vb[q] = lo ? make_double2(y0.x - y1.y, y0.y + y1.x) : make_double2(y0.x + y1.y, y1.x - y0.y);
+        }
+        XPass2<N, true, 0, 1>::run(va, vb, bufA, bufB, i, team, stw, wr);
+        const double s = a.scale;
+#pragma unroll
+        for (int m = 0; m < E / RL; ++m)
+#pragma unroll
+            for (int q = 0; q < RL; ++q) {
+                const int x = i + TP * (m + q * (E / RL));
+                if (oka) { ra0[x] = va[m * RL + q].x * s; ra1[x] = va[m * RL + q].y * s; }
+                if (okb) { rb0[x] = vb[m * RL + q].x * s; rb1[x] = vb[m * RL + q].y * s; }
+            }
+    }
+}
+
 // Lengths 3*2^a (12 or 24 points per thread, a radix-3 last pass): the same team machinery with one exchange buffer per
 // team and general first/last-pass index sets.  128 threads per CTA (4 teams at N = 768), persistent.
 template <int N> struct XRowGenCfg {
@@ -542,6 +653,24 @@ template <int N> static cudaError_t launch_xrows_n(bool inverse, const RowArgs& 
             if (e == cudaSuccess) e = cudaFuncSetAttribute(xrows_kernel<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RC::SMEM);
             if (e != cudaSuccess) return e;
             once.done[dev] = true;
+        }
+        if constexpr (MHD_XROWS_INV_STAGED && N >= 256) {
+            using SC = XRowStagedCfg<N>;
+            const size_t smem = SC::smem(a.spec_pitch);
+            // (bulk copies want 16-byte aligned rows: any complex pitch is; the array itself comes from a 256-byte aligned workspace)
+            if (inverse && smem <= (size_t)227 * 1024 && a.nrows % 2 == 0 && ((size_t)a.spec & 15u) == 0) {
+                static DeviceOnce once_staged;
+                if (!once_staged.done[dev]) {
+                    e = cudaFuncSetAttribute(xrows_inv_staged_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+                    if (e != cudaSuccess) return e;
+                    once_staged.done[dev] = true;
+                }
+                const long long units = (((a.nrows + 1) / 2 + 1) / 2 + SC::TEAMS - 1) / SC::TEAMS;
+                const unsigned nb = (unsigned)(units < sms ? units : sms);         // one persistent CTA per SM
+                xrows_inv_staged_kernel<N><<<nb, SC::THREADS, smem, st>>>(a, tw);
+                count_launch();
+                return cudaGetLastError();
+            }
         }
         const long long groups = (((a.nrows + 1) / 2 + 1) / 2 + RC::TEAMS - 1) / RC::TEAMS;   // two row pairs per team iteration
         const long long cap = (long long)sms * 8;             // persistent; more CTAs than can be resident simply queue
