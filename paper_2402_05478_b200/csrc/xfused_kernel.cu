@@ -405,13 +405,16 @@ __global__ void __launch_bounds__(XRowCfg<N>::THREADS) xrows_kernel(RowArgs a, c
     }
 }
 
-// Inverse x rows with TMA-staged inputs (N >= 256, 8 points per thread): the plain inverse kernel above spends its time waiting
+// Inverse x rows with TMA-staged inputs (N >= 128, 8 points per thread): the plain inverse kernel above spends its time waiting
 // for its row loads (ncu: long scoreboard, 56 % of the DRAM rate against 78 % for the forward direction).  Here one persistent
 // CTA per SM runs the fused pass's scheme: a team's NEXT unit (four consecutive half-spectrum rows = one contiguous block) is
 // brought into shared memory by one bulk copy (cp.async.bulk + mbarrier, two staging buffers per team) while the current unit
 // is transformed, so no warp ever waits on a global load.
 #ifndef MHD_XROWS_INV_STAGED
 #define MHD_XROWS_INV_STAGED 1
+#endif
+#ifndef MHD_XROWS_INV_STAGED_MIN
+#define MHD_XROWS_INV_STAGED_MIN 128     // shortest row length that takes the staged kernel
 #endif
 template <int N> struct XRowStagedCfg {
     static constexpr int TP = Plan<N>::TP;
@@ -654,7 +657,7 @@ template <int N> static cudaError_t launch_xrows_n(bool inverse, const RowArgs& 
             if (e != cudaSuccess) return e;
             once.done[dev] = true;
         }
-        if constexpr (MHD_XROWS_INV_STAGED && N >= 256) {
+        if constexpr (MHD_XROWS_INV_STAGED && N >= MHD_XROWS_INV_STAGED_MIN) {
             using SC = XRowStagedCfg<N>;
             const size_t smem = SC::smem(a.spec_pitch);
             // (bulk copies want 16-byte aligned rows: any complex pitch is; the array itself comes from a 256-byte aligned workspace)
