@@ -159,6 +159,35 @@ enum { MHD_FFT_THREE_SWEEP = 0, MHD_FFT_PLANE_PIPELINE = 1 };
 int mhd_fft_plan_set_mode(mhd_fft_plan* plan, int mode);
 const char* mhd_fft_last_error(const mhd_fft_plan* plan);   /* detail of the last MHD_ECUDA on this plan ("" if none) */
 
+/* ---- The inverse transform without a workspace -------------------------------------------------------------------
+ * mhd_fft_c2r computes out = C2R(in) through a plan, and a plan needs device memory from the caller (twiddle tables and one
+ * half-spectrum-sized intermediate, since `in` is never written).  A caller that owns its input and output and cannot get
+ * any more device memory -- a callback inside a framework whose allocator already holds the whole GPU, a job whose fixed
+ * memory budget is fully handed out, a loop that may not call cudaMalloc because cudaMalloc synchronises the device --
+ * calls this instead.  Same transform, same layouts, same kernels and twiddle values as mhd_fft_c2r (plan of nx, ny, nz,
+ * batch in the default three-sweep mode): in_complex_dev [batch][nz][ny][nx/2+1] complex, read only; out_real_dev
+ * [batch][nz][ny][nx] doubles; includes 1/(nx*ny*nz).  Both are DEVICE pointers on the same GPU; the call runs on the GPU
+ * that owns out_real_dev, enqueued on cuda_stream (NULL = legacy default stream), and is asynchronous after the first call.
+ *
+ * The scratch is an array compiled into the library: MHD_STATIC_SCRATCH_BYTES for the intermediate plus 56 KiB of twiddle
+ * tables.  Every GPU that loads the library holds it until the process exits, used or not, which is why it is small.
+ * The call allocates and frees nothing on the device.  A transform whose intermediate, 16*(nx/2+1)*ny*nz*batch bytes,
+ * exceeds MHD_STATIC_SCRATCH_BYTES (64^3 x 3, 96^3, 512^2 x 3 fit; 128^3 does not) is refused with MHD_EINVAL before
+ * anything is launched, and err_host says how much was asked for and how much there is.
+ *
+ * First call on each GPU: looks up the array's device address, uploads the twiddle tables and synchronises cuda_stream
+ * (a few hundred microseconds).  Make that call before you begin any stream capture on that GPU; a 8x8x8 transform will do.
+ * One array per GPU, shared by every call: two calls that can run at the same time on one GPU (different streams, or
+ * different host threads without a common stream) overwrite each other's intermediate -- keep them on one stream or order
+ * them yourself.  The array keeps the previous call's contents; nothing in it has to start at zero, because every element a
+ * call reads it has written earlier in the same call, so nothing is cleared.
+ *
+ * err_host: optional HOST buffer of err_bytes for a one-line description of a failure ("" on success); may be NULL.
+ * Returns MHD_OK, MHD_EINVAL (unsupported length, NULL buffer, too large) or MHD_ECUDA. */
+#define MHD_STATIC_SCRATCH_BYTES (8u << 20)
+int mhd_fft_c2r_static(int nx, int ny, int nz, int batch, const double* in_complex_dev, double* out_real_dev,
+                       void* cuda_stream, char* err_host, size_t err_bytes);
+
 /* ==== Instrumentation (not part of the solver's contract; used by bench.py and the tests) ====================== */
 
 /* number of kernel launches this library has enqueued since load (bench.py's gpu_launches) */

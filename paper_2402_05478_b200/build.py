@@ -19,7 +19,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libmhd_b200.so")
 OBJDIR = os.path.join(HERE, "build")
 SOURCES = ["fft_kernels.cu", "xfused_kernel.cu", "planefft_kernel.cu", "mhd_kernels.cu", "peaks_kernel.cu",
-           "mhd_api.cu"]
+           "mhd_api.cu", "fft_c2r_static.cu"]
 HEADERS = ["fft_core.cuh", "xteam.cuh", "bulk_copy.cuh", "mhd_internal.h"]
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

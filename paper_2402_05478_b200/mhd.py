@@ -18,6 +18,7 @@ AB2, RK4 = 0, 1
 FLAG_HYDRO, FLAG_NO_DEALIAS, FLAG_FORCING = 1, 2, 4
 FLAG_UNFUSED_X, FLAG_NO_GRAPH = 8, 16
 FFT_THREE_SWEEP, FFT_PLANE_PIPELINE = 0, 1
+STATIC_SCRATCH_BYTES = 8 << 20          # MHD_STATIC_SCRATCH_BYTES: largest intermediate fft_c2r_static accepts
 
 EXPORTS = [
     "mhd_workspace_bytes", "mhd_create", "mhd_destroy", "mhd_set_fields", "mhd_set_fields_host", "mhd_set_box",
@@ -25,6 +26,7 @@ EXPORTS = [
     "mhd_state_bytes", "mhd_get_state", "mhd_set_state",
     "mhd_get_fields", "mhd_get_fields_host", "mhd_diagnostics", "mhd_strerror", "mhd_last_error",
     "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy", "mhd_fft_last_error", "mhd_fft_plan_set_mode",
+    "mhd_fft_c2r_static",
     "mhd_launch_count", "mhd_profile_kernel_count", "mhd_profile_kernel_name", "mhd_profile_begin", "mhd_profile_end",
     "mhd_measure_peaks", "mhd_measure_exchange",
 ]
@@ -87,6 +89,7 @@ def lib():
         L.mhd_fft_plan_set_mode.argtypes = [_vp, C.c_int]
         L.mhd_fft_last_error.restype = C.c_char_p
         L.mhd_fft_last_error.argtypes = [_vp]
+        L.mhd_fft_c2r_static.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, C.c_char_p, C.c_size_t]
         L.mhd_launch_count.restype = C.c_longlong
         L.mhd_profile_kernel_count.restype = C.c_int
         L.mhd_profile_kernel_name.restype = C.c_char_p
@@ -409,3 +412,35 @@ class FftPlan:
             self.close()
         except Exception:
             pass
+
+
+def fft_c2r_static(spec, out=None, stream=None):
+    """mhd_fft_c2r_static: the inverse transform of FftPlan.c2r for code that cannot give the library a workspace.
+
+    FftPlan allocates a workspace tensor; this call allocates nothing on the GPU once `out` is given.  It is meant for
+    callers that own their input and output and no other device memory (a hook inside a framework whose allocator holds the
+    whole GPU, a job with a fully assigned memory budget, a loop that must not hit cudaMalloc's device synchronisation).
+    The scratch is a fixed array inside the library: the transform's intermediate, 16 bytes per element of `spec`, may not
+    exceed STATIC_SCRATCH_BYTES (8 MiB), else MhdError says how much was asked for.
+
+    spec: contiguous CUDA complex128 tensor [batch][nz][ny][nx/2+1] (nx is taken as 2*(last dim - 1)); out: contiguous CUDA
+    float64 tensor [batch][nz][ny][nx] on the same GPU (created with torch.empty when None -- pass it if you cannot
+    allocate).  Enqueued on `stream` (default: the current torch stream of spec's device).  The first call on a GPU also
+    sets the scratch up and synchronises the stream: make it before any stream capture.  All calls on one GPU share the
+    scratch, so calls on different streams must not overlap."""
+    torch = _torch()
+    if not (isinstance(spec, torch.Tensor) and spec.is_cuda and spec.dtype == torch.complex128 and spec.is_contiguous() and spec.dim() == 4):
+        raise ValueError("spec: expected a contiguous CUDA complex128 tensor [batch][nz][ny][nx/2+1]")
+    batch, nz, ny, nxh = (int(v) for v in spec.shape)
+    nx = 2 * (nxh - 1)
+    if out is None:
+        out = torch.empty((batch, nz, ny, nx), dtype=torch.float64, device=spec.device)
+    if out.device != spec.device:
+        raise ValueError("out: must live on the same GPU as spec")
+    optr = _dev_ptr(out, batch * nz * ny * nx, "out")
+    s = torch.cuda.current_stream(spec.device) if stream is None else stream
+    err = C.create_string_buffer(256)
+    rc = lib().mhd_fft_c2r_static(nx, ny, nz, batch, _vp(spec.data_ptr()), optr, _vp(s.cuda_stream), err, len(err))
+    if rc != OK:
+        raise MhdError(rc, "mhd_fft_c2r_static", err.value.decode())
+    return out
