@@ -22,15 +22,30 @@ FLAG_HYDRO, FLAG_NO_DEALIAS = 1, 2
 FIELD_NAMES = ("rho", "mx", "my", "mz", "bx", "by", "bz")
 
 
+_SAN_LIB = os.path.join(_HERE, "libmhd_ref_san.so")
+
+
+def sanitize() -> bool:
+    """MHD_REF_SANITIZE=1: the oracle built with AddressSanitizer + UndefinedBehaviourSanitizer.  The process
+    must then be started with libasan preloaded, e.g.
+        MHD_REF_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+            python -m pytest tests -m "not gpu" -q
+    (the interpreter itself is not instrumented, so leak detection is switched off).  Test infrastructure only."""
+    return os.environ.get("MHD_REF_SANITIZE", "") not in ("", "0")
+
+
 def build(force: bool = False) -> str:
     """Compile oracle/mhd_ref.c into oracle/libmhd_ref.so with gcc (building the checker is not using it)."""
-    stale = (not os.path.exists(_LIB)) or any(
-        os.path.getmtime(p) > os.path.getmtime(_LIB) for p in (_SRC, _HDR))
+    lib_path = _SAN_LIB if sanitize() else _LIB
+    stale = (not os.path.exists(lib_path)) or any(
+        os.path.getmtime(p) > os.path.getmtime(lib_path) for p in (_SRC, _HDR))
     if force or stale:
-        cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-fcx-limited-range",
-               "-Wall", "-Wextra", "-o", _LIB, _SRC, "-lm"]
+        opt = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] \
+            if sanitize() else ["-O2"]
+        cmd = ["gcc"] + opt + ["-std=c99", "-fPIC", "-shared", "-fopenmp", "-fcx-limited-range",
+                               "-Wall", "-Wextra", "-o", lib_path, _SRC, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
-    return _LIB
+    return lib_path
 
 
 class Diag(C.Structure):
