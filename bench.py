@@ -80,19 +80,30 @@ def algorithmic_bytes(g, hydro=False):
     return b
 
 
+# radices of the fused x pass per length, in execution order: the Plan<N> table of csrc/fft_core.cuh (8 points per thread)
+XFUSED_RADICES = {8: (8,), 16: (8, 2), 32: (8, 4), 64: (8, 8), 128: (8, 4, 4), 256: (8, 8, 4), 512: (8, 8, 8),
+                  1024: (8, 8, 4, 4)}
+BUTTERFLY_FP64 = {8: 56, 4: 16, 2: 4}        # FP64 instructions of one radix-r butterfly (fft_core.cuh bfly8 / bfly4 / bfly2)
+
+
 def xfused_onchip_model(g, hydro=False):
     """On-chip work of one x_fused launch that no implementation of this design can avoid:
-    per (z,y) row 4 inverse + 6 forward complex transforms of length nx (two real rows share one), each log8(nx) radix-8
-    passes of nx/8 butterflies: 56 FP64 instructions per butterfly + 28 for the 7 twiddle multiplications of every pass
-    but the first; ~35 FP64 instructions per grid point for the products; between passes every complex (16 B) is written to
-    and read from shared memory once.  Returns (FP64 instruction slots, shared-memory bytes) per launch."""
-    import math
+    per (z,y) row 4 inverse + 6 forward complex transforms of length nx (two real rows share one); every pass of radix r is
+    nx/r butterflies (56 / 16 / 4 FP64 instructions for r = 8 / 4 / 2) and, on every pass but the first, r-1 twiddle
+    multiplications of 4 instructions per butterfly; ~35 FP64 instructions per grid point for the products; between passes
+    every complex (16 B) is written to and read from shared memory once.  The radices are the kernel's own plan table
+    (XFUSED_RADICES), so 128 = 8*4*4 counts 3 passes and 1024 = 8*8*4*4 counts 4.
+    Returns (FP64 instruction slots, shared-memory bytes) per launch; raises for a length the fused pass does not take."""
     nx = g["nx"]
+    if nx not in XFUSED_RADICES:
+        raise ValueError(f"the fused x pass has no plan for nx = {nx}")
+    radices = XFUSED_RADICES[nx]
     rows = g["ny"] * g["nz"]
     nfft = (2 + 5) if hydro else (4 + 6)
-    passes = max(1, round(math.log(nx, 8)))                 # 512 -> 3 (lengths that are not powers of 8: nearest count)
-    bf = nx // 8
-    dp_fft = bf * (56 * passes + 28 * (passes - 1))
+    passes = len(radices)
+    dp_fft = 0
+    for s_, r in enumerate(radices):
+        dp_fft += (nx // r) * (BUTTERFLY_FP64[r] + (4 * (r - 1) if s_ > 0 else 0))
     dp = rows * (nfft * dp_fft + 35 * nx)
     smem = rows * (nfft * (passes - 1) * 2 * 16 * nx          # exchanges: store + load of every complex
                    + (4 if hydro else 7) * 16 * g["nkx"]      # staged input rows read once
@@ -193,22 +204,52 @@ def time_oracle(n, steps, warmup, threads=None):
     return dt / steps, cores
 
 
+def host_ram_available_gb():
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable:"):
+                return int(line.split()[1]) / 2 ** 20
+    except (OSError, ValueError):
+        pass
+    return 0.0
+
+
+ORACLE_512_GB = 80.0     # the oracle's arrays at 512^3 (about 57 GB) + the input fields, with headroom
+
+
+def oracle_sample_grid(requested, total_steps, budget_s=240.0):
+    """Grid of the bounded oracle sample.  BASELINE.md §4 asks for the metric's own grid (512^3): taken when the host has the
+    memory and `total_steps` oracle steps fit the time budget (about 17 s per step at 512^3 and 2.1 s at 256^3 on the
+    16 host cores of a B200 box); otherwise 256^3, then 128^3.  Returns (n, reason)."""
+    if requested:
+        return int(requested), "grid requested on the command line"
+    avail = host_ram_available_gb()
+    if avail >= ORACLE_512_GB and total_steps * 17.0 <= budget_s:
+        return 512, "the metric's own grid"
+    why = (f"only {avail:.0f} GB of host memory available (512^3 needs about {ORACLE_512_GB:.0f})" if avail < ORACLE_512_GB
+           else f"{total_steps} oracle steps at 512^3 would take about {total_steps * 17.0:.0f} s")
+    if total_steps * 2.1 <= budget_s:
+        return 256, why
+    return 128, why
+
+
 # ------------------------------------------------------------------------------------------------
 def run_reference(args):
     """--impl reference: the oracle on the host cores (rank 0 only; other ranks exit 0 without work)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return 0
-    n = args.ref_n
+    n, why = oracle_sample_grid(args.ref_n, args.steps + args.warmup)
     sec, cores = time_oracle(n, args.steps, args.warmup)
     value = n ** 3 / sec
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"config4 recipe (decaying MHD turbulence, AB2, 2/3 dealiasing) on a bounded {n}^3 sample of the 512^3 box",
-                   "grid": [n, n, n], "integrator": "AB2"},
+        "config": {"workload": (f"config4: 3D MHD decaying turbulence {n}^3, AB2, 2/3 dealiasing, nu=eta=1e-3, dt=2e-4, cs=1" if n == 512 else
+                                f"config4 recipe (decaying MHD turbulence, AB2, 2/3 dealiasing) on a bounded {n}^3 sample of the 512^3 box"),
+                   "grid": [n, n, n], "integrator": "AB2", "grid_choice": why},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": f"{args.steps} AB2 steps at {n}^3 after {args.warmup} warm-up steps"},
+                         "sample": f"{args.steps} AB2 steps at {n}^3 after {args.warmup} warm-up steps ({why})"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -304,40 +345,41 @@ def run_gpu(args):
              "algorithmic_gb": abytes[name] / 1e9, "gbs": abytes[name] / 1e9 / (per * 1e-3),
              "hbm_frac": abytes[name] / 1e9 / (per * 1e-3) / peak, "share_of_step": ms / ms_prof_total,
              "traffic": traffic.get(name)}
+        # ALGORITHMIC floors only: bytes the method must move, FP64 instructions the method must issue.
         floors = {"hbm": abytes[name] / (peak * 1e9) * 1e3}               # ms
         if name == "x_fused":
             dp, smem = xfused_onchip_model(geo)
             floors["alu"] = dp * 2.0 / (fp64_tflops * 1e12) * 1e3          # every FP64 instruction occupies one DFMA slot (2 flop)
-            floors["smem"] = smem / (smem_gbs * 1e9) * 1e3
             k["fp64_instr"] = dp
-            k["smem_bytes"] = smem
-            k["smem_exchange_ceiling_gbs"] = exch_gbs
-            k["frac_of_exchange_ceiling"] = smem / 1e9 / (per * 1e-3) / exch_gbs if exch_gbs > 0 else None
+            # this implementation's own shared-memory traffic (two exchanges per transform through padded buffers): a property
+            # of the design, not of the method -- a diagnostic, never the roofline
+            smem_gbs_kernel = smem / 1e9 / (per * 1e-3)
+            k["design_model"] = {"smem_bytes": smem, "smem_floor_ms": smem / (smem_gbs * 1e9) * 1e3,
+                                 "frac_of_smem_peak": smem_gbs_kernel / smem_gbs if smem_gbs > 0 else None,
+                                 "smem_exchange_ceiling_gbs": exch_gbs,
+                                 "frac_of_exchange_ceiling": smem_gbs_kernel / exch_gbs if exch_gbs > 0 else None}
         k["floors_ms"] = floors
         k["bound"] = max(floors, key=floors.get)
         k["frac"] = floors[k["bound"]] / per
         kernels.append(k)
     kernels.sort(key=lambda k: -k["share_of_step"])
     top = kernels[0]
-    unit = {"hbm": "GB/s", "alu": "TFLOP/s", "smem": "GB/s"}[top["bound"]]
+    unit = {"hbm": "GB/s", "alu": "TFLOP/s"}[top["bound"]]
     if top["bound"] == "hbm":
         achieved, pk, what = top["gbs"], peak, peak_src
-    elif top["bound"] == "alu":
+    else:
         achieved, pk = top["fp64_instr"] * 2.0 / 1e12 / (top["ms_per_launch"] * 1e-3), fp64_tflops
         what = "measured in this run by mhd_measure_peaks (independent DFMA chains; a DFMA slot = 2 flop)"
-    else:
-        achieved, pk = top["smem_bytes"] / 1e9 / (top["ms_per_launch"] * 1e-3), smem_gbs
-        what = "measured in this run by mhd_measure_peaks (conflict-free 16-byte shared-memory stores + loads)"
     roofline = {"bound": top["bound"], "kernel": top["kernel"], "achieved": achieved, "peak": pk, "unit": unit,
                 "frac": top["frac"], "traffic": top["traffic"], "peak_source": what,
                 "hbm_frac": top["hbm_frac"], "hbm_peak": peak, "hbm_peak_source": peak_src,
-                "smem_exchange_ceiling_gbs": top.get("smem_exchange_ceiling_gbs"), "frac_of_exchange_ceiling": top.get("frac_of_exchange_ceiling"),
                 "algorithmic_bytes_per_launch": abytes[top["kernel"]], "floors_ms": top["floors_ms"],
-                "share_of_step": top["share_of_step"],
-                "note": "bound = the highest of the kernel's floors (HBM bytes, FP64 instruction slots, shared-memory bytes; models in "
-                        "DESIGN.md §6); frac = that floor / measured time; hbm_frac is kept beside it; smem_exchange_ceiling_gbs = what "
-                        "the kernel's own barrier-synchronised exchange pattern reaches with everything else stripped away "
-                        "(mhd_measure_exchange), frac_of_exchange_ceiling = the kernel's shared-memory GB/s over that"}
+                "share_of_step": top["share_of_step"], "design_model": top.get("design_model"),
+                "note": "bound = the higher of the kernel's ALGORITHMIC floors (HBM bytes of the pruned transforms; FP64 instruction "
+                        "slots of the butterflies and products, DESIGN.md §6); frac = that floor / measured time; hbm_frac is kept "
+                        "beside it.  design_model = this implementation's own shared-memory traffic against the measured "
+                        "shared-memory peak and against what its barrier-synchronised exchange pattern reaches alone "
+                        "(mhd_measure_exchange): a diagnostic of the design, not a roofline"}
     own_bytes = sum(k["algorithmic_gb"] * 1e9 * k["launches_per_step"] for k in kernels)   # only the kernel classes that ran
     step_roofline = {
         "design_bytes_per_step": own_bytes, "design_gbs": own_bytes / 1e9 / (ms_step * 1e-3),
@@ -357,9 +399,13 @@ def run_gpu(args):
     # ---- the oracle timed beside it on this box's host cores (bounded sample) ----
     cpu = None
     if not args.no_cpu_baseline:
-        sec, cores = time_oracle(args.cpu_n, args.cpu_steps, 1)
-        cpu = {"value": args.cpu_n ** 3 / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{args.cpu_steps} AB2 steps (after 1 Euler warm-up step) of the config-4 recipe at {args.cpu_n}^3, {sec:.2f} s per step"}
+        host = None                                  # the pinned input copies (7 fields) are no longer needed
+        import gc
+        gc.collect()
+        cpu_n, why = oracle_sample_grid(args.cpu_n, args.cpu_steps + 1, budget_s=90.0)
+        sec, cores = time_oracle(cpu_n, args.cpu_steps, 1)
+        cpu = {"value": cpu_n ** 3 / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{args.cpu_steps} AB2 steps (after 1 Euler warm-up step) of the config-4 recipe at {cpu_n}^3 ({why}), {sec:.2f} s per step"}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_step,
@@ -462,7 +508,7 @@ def fft_sweep_rows(sizes, dev, peak, reps=5, cufft=True):
         batch = 7
         gen = torch.Generator(device=dev); gen.manual_seed(1005)
         a = torch.rand((batch, n, n, n), dtype=torch.float64, device=dev, generator=gen) * 2.0 - 1.0
-        plan = mhd.FftPlan(n, n, n, batch, stream=torch.cuda.current_stream(dev))
+        plan = mhd.FftPlan(n, n, n, batch, stream=torch.cuda.current_stream(dev), plane_workspace=n in (64, 128, 256, 512))
         spec = plan.r2c(a)
         back = plan.c2r(spec)
         err = float(torch.linalg.norm(back - a) / torch.linalg.norm(a))
@@ -546,9 +592,9 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--n", type=int, default=512, help="grid size of the timed workload (config 4 is 512)")
-    ap.add_argument("--ref-n", type=int, default=128, help="grid size of the bounded sample the reference arm times")
-    ap.add_argument("--cpu-n", type=int, default=256, help="grid size of the bounded cpu_baseline sample")
-    ap.add_argument("--cpu-steps", type=int, default=4, help="timed oracle steps of the cpu_baseline sample (about 10-20 s of CPU work)")
+    ap.add_argument("--ref-n", type=int, default=0, help="grid size the reference arm times (0: 512 when memory and the step count allow, else 256 / 128)")
+    ap.add_argument("--cpu-n", type=int, default=0, help="grid size of the cpu_baseline sample (0: 512, the metric's grid, when the host has the memory, else 256)")
+    ap.add_argument("--cpu-steps", type=int, default=3, help="timed oracle steps of the cpu_baseline sample (BASELINE.md §4: 3 steps at 512^3, about 60 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="step", choices=["step", "fft", "peaks"],
                     help="step: the 512^3 MHD step (default, carries the compact FFT sweep too); fft: the config-5 FFT sweep with the cuFFT line; "

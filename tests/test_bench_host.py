@@ -55,7 +55,17 @@ def test_xfused_onchip_model_matches_the_design_derivation():
     alu_ms, smem_ms, hbm_ms = dp * 2 / 34.1e12 * 1e3, smem / 36.5e12 * 1e3, bench.algorithmic_bytes(g)["x_fused"] / 6542.1e9 * 1e3
     assert 2.3 < alu_ms < 2.6 and 2.6 < smem_ms < 2.9 and 2.0 < hbm_ms < 2.2
     dph, _ = bench.xfused_onchip_model(bench.geometry(256, 256, 1), hydro=True)
-    assert dph == 256 * (7 * 32 * (56 * 3 + 28 * 2) + 35 * 256)      # log8(256) rounds to 3 passes; 2 inverse + 5 forward transforms
+    # 256 = 8*8*4 (the kernel's plan): two radix-8 passes of 32 butterflies, one radix-4 pass of 64; 2 inverse + 5 forward transforms
+    assert dph == 256 * (7 * (32 * 56 + 32 * (56 + 28) + 64 * (16 + 12)) + 35 * 256)
+    # lengths that are not powers of 8 take their pass count from the plan table, not from log8: 128 = 8*4*4, 1024 = 8*8*4*4
+    dp128, sm128 = bench.xfused_onchip_model(bench.geometry(128, 128, 128))
+    assert dp128 == 128 * 128 * (10 * (16 * 56 + 32 * (16 + 12) * 2) + 35 * 128)
+    assert sm128 == 128 * 128 * (10 * 2 * 2 * 16 * 128 + 7 * 16 * 43 + 6 * 2 * 16 * 43)
+    dp1024, sm1024 = bench.xfused_onchip_model(bench.geometry(1024, 8, 8))
+    assert dp1024 == 64 * (10 * (128 * 56 + 128 * (56 + 28) + 256 * (16 + 12) * 2) + 35 * 1024)
+    assert sm1024 == 64 * (10 * 3 * 2 * 16 * 1024 + 7 * 16 * 342 + 6 * 2 * 16 * 342)
+    with pytest.raises(ValueError):
+        bench.xfused_onchip_model(bench.geometry(384, 8, 8))         # 3*2^a lengths run the unfused plan
 
 
 def test_parse_clock_samples():
