@@ -89,6 +89,9 @@ def test_orszag_tang_2d_energy_exchange_period(gpu):
     printed = GOLD["period_2d_orszag_tang"]["value"]
     print(f"2-D OT exchange period {T:.4f}; pi/(k0 V_A) = {np.pi:.4f}; printed {printed} ({100 * (T - printed) / printed:+.1f} %)")
     assert abs(T - np.pi) <= 0.03 * np.pi, T
+    # loose pin to the paper's own number as well (tests/golden/paper_values.json): this code sits 5-7 % above the printed
+    # 2.971 for every reading tried, so 8 % holds today and a drift away from the paper's value still fails
+    assert abs(T - printed) <= 0.08 * printed, (T, printed)
     assert d["max_divb"] <= 1e-10
 
 
