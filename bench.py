@@ -396,6 +396,17 @@ def run_gpu(args):
         torch.cuda.empty_cache()
         fft = fft_sweep_rows([int(v) for v in args.fft_sizes.split(",")], dev, peak, reps=3, cufft=False)
 
+    # ---- BASELINE configs 1-3 (launch-bound, L2-resident grids) at full length, AB2, in the same line ----
+    small = None
+    if not args.no_small:
+        from paper_2402_05478_b200 import inputs as _inputs
+        small = []
+        for cid, make in ((1, _inputs.config1), (2, _inputs.config2), (3, _inputs.config3)):
+            c = make()
+            row = time_small_config(c, dev, 2, args.flags, (("AB2", mhd.AB2),))[0]
+            row.update({"config": cid, "grid": [c.nx, c.ny, c.nz], "hydro": bool(c.hydro)})
+            small.append(row)
+
     # ---- the oracle timed beside it on this box's host cores (bounded sample) ----
     cpu = None
     if not args.no_cpu_baseline:
@@ -419,30 +430,25 @@ def run_gpu(args):
         "roofline": roofline, "step_roofline": step_roofline, "kernels": kernels,
         "peaks": {"hbm_gbs": peak, "hbm_source": peak_src, "fp64_tflops": fp64_tflops, "smem_gbs": smem_gbs,
                   "smem_exchange_gbs": exch_gbs, "onchip_source": "mhd_measure_peaks / mhd_measure_exchange(192), this run"},
-        "fft": fft, "cpu_baseline": cpu,
+        "fft": fft, "small_configs": small, "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
     return 0
 
 
-def run_small_config(args):
-    """--config 1|2|3: BASELINE configs 1-3 at their full step count on the shipped path (CUDA-graph replay), AB2, with the
-    oracle timed beside it at FULL length on the host cores (BASELINE.md §4).  These grids are L2-resident and launch-bound."""
+def time_small_config(cfg, dev, reps, extra_flags, integrators):
+    """One BASELINE small config at its full step count on the shipped path (CUDA-graph replay), per integrator: median of
+    `reps` timed runs after one untimed run, CUDA events on the solver's stream."""
     import torch
-    from paper_2402_05478_b200 import inputs, mhd
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device")
-    dev = torch.device("cuda", 0)
-    torch.cuda.set_device(dev)
-    cfg = {1: inputs.config1, 2: inputs.config2, 3: inputs.config3}[args.config]()
-    flags = (mhd.FLAG_HYDRO if cfg.hydro else 0) | args.flags
+    from paper_2402_05478_b200 import mhd
+    flags = (mhd.FLAG_HYDRO if cfg.hydro else 0) | extra_flags
     rows = []
-    for integ, name in ((mhd.AB2, "AB2"), (mhd.RK4, "RK4")):
+    for name, integ in integrators:
         s = mhd.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, integrator=integ, flags=flags, device=dev)
         arrs = [torch.from_numpy(a).to(dev) for a in cfg.arrays()]
         ts = []
         l0 = mhd.launch_count()
-        for rep in range(1 + args.reps):
+        for rep in range(1 + reps):
             s.set_fields(*arrs)
             s.step(4)                                   # Euler start, eager step, capture, first replay: not timed
             s.synchronize()
@@ -455,8 +461,22 @@ def run_small_config(args):
         d = s.diagnostics(0)
         rows.append({"integrator": name, "steps": cfg.steps, "ms_per_step": ms / cfg.steps,
                      "grid_point_updates_per_s": cfg.nx * cfg.ny * cfg.nz * cfg.steps / (ms * 1e-3),
-                     "launches": (mhd.launch_count() - l0) // (1 + args.reps), "ekin": d["ekin"], "emag": d["emag"]})
+                     "launches": (mhd.launch_count() - l0) // (1 + reps), "ekin": d["ekin"], "emag": d["emag"]})
         s.close()
+    return rows
+
+
+def run_small_config(args):
+    """--config 1|2|3: BASELINE configs 1-3 at their full step count on the shipped path (CUDA-graph replay), AB2, with the
+    oracle timed beside it at FULL length on the host cores (BASELINE.md §4).  These grids are L2-resident and launch-bound."""
+    import torch
+    from paper_2402_05478_b200 import inputs, mhd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    cfg = {1: inputs.config1, 2: inputs.config2, 3: inputs.config3}[args.config]()
+    rows = time_small_config(cfg, dev, args.reps, args.flags, (("AB2", mhd.AB2), ("RK4", mhd.RK4)))
     cpu = None
     if not args.no_cpu_baseline:
         from oracle import mhd_ref
@@ -484,7 +504,8 @@ def run_peaks(args):
     vals = [mhd.measure_peaks("cuda:0") for _ in range(3)]
     exch = {str(d): max(mhd.measure_exchange(d, "cuda:0") for _ in range(2)) for d in (0, 64, 128, 192, 256)}
     exch_modes = {name: max(mhd.measure_exchange(192, "cuda:0", m) for _ in range(2))
-                  for m, name in enumerate(("write_barrier_read_barrier", "barrier_write_barrier_read", "double_buffer_one_barrier"))}
+                  for m, name in enumerate(("write_barrier_read_barrier", "barrier_write_barrier_read", "double_buffer_one_barrier",
+                                             "warp_shuffle_octet_transpose_no_smem"))}
     clocks = sampler.stop()
     f, sm = max(v[0] for v in vals), max(v[1] for v in vals)
     sms = torch.cuda.get_device_properties(0).multi_processor_count
@@ -600,6 +621,7 @@ def main(argv=None):
                     help="step: the 512^3 MHD step (default, carries the compact FFT sweep too); fft: the config-5 FFT sweep with the cuFFT line; "
                          "peaks: the measured FP64 / shared-memory ceilings")
     ap.add_argument("--fft-sizes", default="128,256,512,768")
+    ap.add_argument("--no-small", action="store_true", help="skip the BASELINE config 1-3 rows (small_configs) in the default line")
     ap.add_argument("--no-fft", action="store_true", help="skip the compact config-5 sweep in the default line")
     ap.add_argument("--config", type=int, default=0, choices=[0, 1, 2, 3], help="time BASELINE config 1, 2 or 3 at full length instead")
     ap.add_argument("--reps", type=int, default=3, help="--config: timed repetitions (median)")

@@ -79,7 +79,9 @@ size_t mhd_workspace_bytes(int nx, int ny, int nz, int integrator, unsigned flag
  * workspace_dev: caller-owned device memory, 256-byte aligned, >= mhd_workspace_bytes(...), must stay
  * alive and untouched until mhd_destroy.  cuda_stream: a cudaStream_t; NULL = the legacy default
  * stream, on which mhd_step cannot use CUDA graphs (small grids then pay per-launch latency).
- * Errors: MHD_EINVAL (bad size/parameter/NULL/workspace too small), MHD_ENOMEM (host), MHD_ECUDA. */
+ * Errors: MHD_EINVAL (bad size/parameter/NULL/workspace too small, or cuda_stream was created on another GPU than the one
+ * that owns the workspace), MHD_ENOMEM (host), MHD_ECUDA.  Any later call returns MHD_ECUDA, without launching anything, if
+ * the GPU that owns the workspace cannot be made current. */
 int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, double cs, double dt,
                int integrator, unsigned flags, void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 void mhd_destroy(mhd_ctx* ctx);
@@ -157,6 +159,11 @@ void mhd_fft_plan_destroy(mhd_fft_plan* plan);
  * the two separate passes (profiles/r02_planefft.md): hence not the default. */
 enum { MHD_FFT_THREE_SWEEP = 0, MHD_FFT_PLANE_PIPELINE = 1 };
 int mhd_fft_plan_set_mode(mhd_fft_plan* plan, int mode);
+/* The plane pipeline needs a ring of plane groups and its counters behind the plan's ordinary workspace (about 20 MB).  Only a
+ * plan that will use it pays: mhd_fft_workspace_bytes does not include them; a plan created on at least
+ * mhd_fft_plane_workspace_bytes(...) bytes (0 for shapes the mode does not take) may switch to MHD_FFT_PLANE_PIPELINE, any
+ * smaller plan gets MHD_EINVAL from mhd_fft_plan_set_mode. */
+size_t mhd_fft_plane_workspace_bytes(int nx, int ny, int nz, int batch);
 const char* mhd_fft_last_error(const mhd_fft_plan* plan);   /* detail of the last MHD_ECUDA on this plan ("" if none) */
 
 /* ---- The inverse transform without a workspace -------------------------------------------------------------------
@@ -214,7 +221,10 @@ int mhd_measure_peaks(void* scratch_dev, size_t scratch_bytes, void* cuda_stream
 /* What the fused x pass's own shared-memory exchange pattern reaches with everything else stripped away: 4 teams of 64 threads
  * per SM, per iteration dfma_per_exchange (0, 64, 128, 192 or 256) independent DFMAs per thread, then 16 STS.128 and 16 LDS.128
  * (the padded index sets of the Stockham passes) with team barriers placed by barrier_mode: 0 = write, barrier, read, barrier;
- * 1 = barrier, write, barrier, read (the shipped x passes); 2 = two buffers used alternately, one barrier per exchange.
+ * 1 = barrier, write, barrier, read (the shipped x passes); 2 = two buffers used alternately, one barrier per exchange;
+ * 3 = no shared memory at all: the same 16 complex values per thread exchanged by an 8 x 8 register transpose among the 8 lanes
+ * of a warp octet (three __shfl_xor_sync rounds) -- the upper bound of a warp-shuffle exchange, reported in the same unit
+ * (512 bytes per thread and exchange) so that it can be read against the shared-memory modes.
  * Result: GB/s moved through shared memory.  The fused pass at N = 512 has ~190 FP64 instructions per thread between
  * exchanges; its achievable ceiling is this number, not the free-running shared-memory peak of mhd_measure_peaks.
  * scratch_dev as above; synchronises; MHD_EINVAL for other counts or modes. */

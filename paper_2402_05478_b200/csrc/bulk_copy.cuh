@@ -1,5 +1,6 @@
-// bulk_copy.cuh — TMA bulk copies (cp.async.bulk, global -> shared) completing on an mbarrier: the asynchronous staging used
-// by the fused x pass (rows) and by the strided-axis FFT kernels (tiles).  No registers are held while the data is in flight.
+// bulk_copy.cuh — TMA bulk copies (cp.async.bulk, global -> shared) completing on an mbarrier: the asynchronous staging of
+// half-spectrum rows used by the fused x pass and by the stand-alone inverse x rows (xfused_kernel.cu).  The strided-axis
+// kernels do not use it (tile staging was measured and not kept).  No registers are held while the data is in flight.
 #pragma once
 #include <cuda_runtime.h>
 

@@ -149,7 +149,13 @@ struct Padded {
 // ---- the passes ----------------------------------------------------------------------------
 // tw[j] = exp(-2*pi*i*j/N), j = 0..N-1 (forward); the inverse conjugates on the fly.
 // sm + lay(e): where element e of this thread's pencil lives between passes.  i: slot (0..TP-1).
-template <int N, bool INV, int S, int P, typename L>
+// SYNC: how the exchange between two passes is synchronised.
+//   0  write, barrier, read, barrier -- always safe: the caller may write the buffer again right after run() returns (loops)
+//   1  the same, without the barrier after the LAST exchange's reads: for callers that never touch the buffer again
+//      (one pencil tile per CTA), one barrier fewer per transform
+//   2  two buffers used alternately (exchange S in buffer S & 1, BUF complex apart), one barrier per exchange: the barrier
+//      of exchange S+1 already orders every read of exchange S before the writes of exchange S+2 into the same buffer
+template <int N, bool INV, int S, int P, typename L, int SYNC = 0, int BUF = 0>
 struct Pass {
     static constexpr int R = Plan<N>::radix(S);
     static constexpr int E = Plan<N>::E;
@@ -185,35 +191,38 @@ struct Pass {
             bfly<R, INV>(&v[m * R]);
             if constexpr (!LAST) {
                 const int j = (b - k) * R + k;
+                cplx* buf = sm + ((SYNC == 2 && (S & 1)) ? BUF : 0);
 #pragma unroll
-                for (int q = 0; q < R; ++q) sm[lay(j + q * P)] = v[m * R + q];
+                for (int q = 0; q < R; ++q) buf[lay(j + q * P)] = v[m * R + q];
             }
         }
         if constexpr (!LAST) {
             constexpr int Rn = Plan<N>::radix(S + 1);
+            const cplx* buf = sm + ((SYNC == 2 && (S & 1)) ? BUF : 0);
             __syncthreads();
 #pragma unroll
             for (int m = 0; m < E / Rn; ++m)
 #pragma unroll
-                for (int q = 0; q < Rn; ++q) v[m * Rn + q] = sm[lay(i + TP * m + q * (N / Rn))];
-            __syncthreads();
-            Pass<N, INV, S + 1, P * R, L>::run(v, sm, i, lay, tw);
+                for (int q = 0; q < Rn; ++q) v[m * Rn + q] = buf[lay(i + TP * m + q * (N / Rn))];
+            constexpr bool next_is_last = (S + 1 == Plan<N>::NP - 1);
+            if constexpr (SYNC == 0 || (SYNC == 1 && !next_is_last)) __syncthreads();
+            Pass<N, INV, S + 1, P * R, L, SYNC, BUF>::run(v, sm, i, lay, tw);
         }
     }
 };
 
 // Transform the pencil whose first-pass inputs are in v (see first_index); on return v holds the
 // last-pass outputs (see last_index).  All threads of the CTA must call it (it synchronises).
-template <int N, bool INV>
+template <int N, bool INV, int SYNC = 0>
 __device__ __forceinline__ void pencil_fft(cplx (&v)[Plan<N>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
     Cols8 lay{p};
-    Pass<N, INV, 0, 1, Cols8>::run(v, sm, i, lay, tw);
+    Pass<N, INV, 0, 1, Cols8, SYNC, N * 8>::run(v, sm, i, lay, tw);
 }
 // same for 4 pencils side by side (lane = (p = tid & 3, slot))
-template <int N, bool INV>
+template <int N, bool INV, int SYNC = 0>
 __device__ __forceinline__ void pencil_fft4(cplx (&v)[Plan<N>::E], cplx* sm, int i, int p, const cplx* __restrict__ tw) {
     Cols4 lay{p};
-    Pass<N, INV, 0, 1, Cols4>::run(v, sm, i, lay, tw);
+    Pass<N, INV, 0, 1, Cols4, SYNC, N * 4>::run(v, sm, i, lay, tw);
 }
 // same, one pencil per (padded) buffer
 template <int N, bool INV>

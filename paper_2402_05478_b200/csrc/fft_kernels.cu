@@ -27,6 +27,11 @@ __device__ __forceinline__ int compact_index(int f, int n, int nk) {
     return -1;
 }
 
+// exchange synchronisation of the strided-axis kernels (fft_core.cuh Pass<..., SYNC>): every CTA transforms ONE tile and exits,
+// so the barrier after the last exchange's reads protects nothing (1); 2 = two buffers, one barrier per exchange
+#ifndef MHD_AXIS_SYNC
+#define MHD_AXIS_SYNC 1
+#endif
 #ifndef MHD_AXIS24_MINB
 #define MHD_AXIS24_MINB 2     // minimum CTAs per SM asked of ptxas for the 24-points-per-thread lengths (0: no request)
 #endif
@@ -52,7 +57,45 @@ __global__ void __launch_bounds__(Tile<N>::THREADS, (Plan<N>::E == 24 ? MHD_AXIS
             const int c = compact_index(first_index<N>(i, m, q), N, a.nk_in);
             v[m * R0 + q] = (colok && c >= 0) ? in[(long long)c * a.in_row] : make_double2(0.0, 0.0);
         }
-    pencil_fft<N, INV>(v, sm, i, p, tw);
+    pencil_fft<N, INV, (MHD_AXIS_SYNC == 2 ? 1 : MHD_AXIS_SYNC)>(v, sm, i, p, tw);      // (two buffers only in the 4-column variant)
+    const double s = a.scale;
+#pragma unroll
+    for (int m = 0; m < PL::E / RL; ++m)
+#pragma unroll
+        for (int q = 0; q < RL; ++q) {
+            const int c = compact_index(last_index<N>(i, m, q), N, a.nk_out);
+            if (colok && c >= 0) out[(long long)c * a.out_row] = make_double2(v[m * RL + q].x * s, v[m * RL + q].y * s);
+        }
+}
+
+// Variant measured in round 3 (profiles/r03_experiments.md): 4 adjacent columns per CTA instead of 8, so a 512-long axis runs
+// in 256-thread CTAs, four per SM, and a __syncthreads stalls 8 warps instead of 16 (64-byte row segments in HBM instead of
+// 128).  Compile-time switch: -DMHD_AXIS_COLS4_MIN=<smallest N that uses it>; 0 (default) = never.
+#ifndef MHD_AXIS_COLS4_MIN
+#define MHD_AXIS_COLS4_MIN 0
+#endif
+template <int N, bool INV>
+__global__ void __launch_bounds__(Plan<N>::TP * 4) fft_axis4_kernel(AxisArgs a, const cplx* __restrict__ tw) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    using PL = Plan<N>;
+    const int tid = threadIdx.x, p = tid & 3, i = tid >> 2;
+    cplx* sm = reinterpret_cast<cplx*>(smraw);
+    const int col = blockIdx.x * 4 + p;
+    const bool colok = col < a.inner;
+    const long long outer = (long long)blockIdx.y + (long long)blockIdx.z * gridDim.y;
+    if (outer >= a.nouter) return;           // uniform per CTA
+    const cplx* __restrict__ in = a.in + outer * a.in_outer + col;
+    cplx* __restrict__ out = a.out + outer * a.out_outer + col;
+    cplx v[PL::E];
+    constexpr int R0 = PL::radix(0), RL = PL::radix(PL::NP - 1);
+#pragma unroll
+    for (int m = 0; m < PL::E / R0; ++m)
+#pragma unroll
+        for (int q = 0; q < R0; ++q) {
+            const int c = compact_index(first_index<N>(i, m, q), N, a.nk_in);
+            v[m * R0 + q] = (colok && c >= 0) ? in[(long long)c * a.in_row] : make_double2(0.0, 0.0);
+        }
+    pencil_fft4<N, INV, MHD_AXIS_SYNC>(v, sm, i, p, tw);
     const double s = a.scale;
 #pragma unroll
     for (int m = 0; m < PL::E / RL; ++m)
@@ -74,9 +117,21 @@ template <int N, bool INV> static cudaError_t launch_axis_n(const AxisArgs& a, c
         if (e != cudaSuccess) return e;
         once.done[dev] = true;
     }
-    const unsigned tiles = (unsigned)((a.inner + Tile<N>::COLS - 1) / Tile<N>::COLS);
     unsigned gy = (unsigned)outer, gz = 1;
     while (gy > 65535u) { gz *= 2; gy = (unsigned)((outer + gz - 1) / gz); }
+    if constexpr (MHD_AXIS_COLS4_MIN > 0 && N >= MHD_AXIS_COLS4_MIN && Plan<N>::E == 8 && Plan<N>::TP * 4 >= 64) {
+        static DeviceOnce once4;
+        constexpr int smem4 = N * 4 * (int)sizeof(cplx) * (MHD_AXIS_SYNC == 2 ? 2 : 1);
+        if (!once4.done[dev]) {
+            cudaError_t e = cudaFuncSetAttribute(fft_axis4_kernel<N, INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem4);
+            if (e != cudaSuccess) return e;
+            once4.done[dev] = true;
+        }
+        fft_axis4_kernel<N, INV><<<dim3((unsigned)((a.inner + 3) / 4), gy, gz), Plan<N>::TP * 4, smem4, st>>>(a, tw);
+        count_launch();
+        return cudaGetLastError();
+    }
+    const unsigned tiles = (unsigned)((a.inner + Tile<N>::COLS - 1) / Tile<N>::COLS);
     fft_axis_kernel<N, INV><<<dim3(tiles, gy, gz), Tile<N>::THREADS, Tile<N>::SMEM, st>>>(a, tw);
     count_launch();
     return cudaGetLastError();

@@ -108,7 +108,7 @@ struct mhd_ctx {
     cudaGraphExec_t graph;     // one steady-state step (AB2 non-first / RK4), replayed by mhd_step
     int graph_ready;
     long long graph_launches;  // kernels inside the captured step
-    int xfuse;                 // fused x pass available for this nx (and not disabled by MHD_NO_XFUSE)
+    int xfuse;                 // fused x pass available for this nx (and not disabled by MHD_FLAG_UNFUSED_X)
     int profiling;             // mhd_profile_begin: eager steps with CUDA events around every kernel
     std::vector<cudaEvent_t>* prof_ev;   // [K_NCLASS] start/stop pairs
     char err[256];
@@ -118,16 +118,31 @@ namespace {
 
 // Makes `device` current for the duration of one API call and restores the caller's device afterwards, so a context
 // (or plan) created on one GPU can be driven while another GPU is current.
+// device < 0 (owner unknown) leaves the caller's device in place by design; a device that is known but cannot be made
+// current sets `failed`, and the API call returns MHD_ECUDA instead of running on the wrong GPU.
 struct DeviceGuard {
     int prev = -1;
     bool switched = false;
+    bool failed = false;
     explicit DeviceGuard(int device) {
-        if (device >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = (cudaSetDevice(device) == cudaSuccess);
+        if (device < 0) return;
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); failed = true; return; }
+        if (prev == device) return;
+        if (cudaSetDevice(device) == cudaSuccess) switched = true;
+        else { cudaGetLastError(); failed = true; }
     }
     ~DeviceGuard() {
         if (switched) cudaSetDevice(prev);
     }
 };
+// a stream created on another GPU than the workspace's cannot carry this context's work (false only when that is certain)
+bool stream_on_device(cudaStream_t st, int device) {
+    if (!st || device < 0) return true;          // legacy default stream: belongs to whichever device is current
+    int sd = -1;
+    if (cudaStreamGetDevice(st, &sd) != cudaSuccess) { cudaGetLastError(); return true; }
+    return sd == device;
+}
+const char* const kGuardFailed = "cannot make the GPU that owns the workspace current";
 // device that owns a device pointer (-1 if it cannot be determined: the current device is then used as is)
 int owning_device(const void* p) {
     cudaPointerAttributes at;
@@ -303,20 +318,23 @@ const char* mhd_profile_kernel_name(int i) { return (i >= 0 && i < K_NCLASS) ? k
 int mhd_measure_peaks(void* scratch, size_t bytes, void* stream, double* fp64_tflops, double* smem_gbs) {
     if (!scratch || !fp64_tflops || !smem_gbs || bytes < ((size_t)4 << 20)) return MHD_EINVAL;
     DeviceGuard guard(owning_device(scratch));
+    if (guard.failed) return MHD_ECUDA;
     return measure_peaks((double*)scratch, bytes / sizeof(double), (cudaStream_t)stream, fp64_tflops, smem_gbs) == cudaSuccess ? MHD_OK : MHD_ECUDA;
 }
 
 int mhd_measure_exchange(void* scratch, size_t bytes, void* stream, int dfma_per_exchange, int barrier_mode, double* smem_gbs) {
     if (!scratch || !smem_gbs || bytes < ((size_t)4 << 20)) return MHD_EINVAL;
     if (dfma_per_exchange < 0 || dfma_per_exchange > 256 || dfma_per_exchange % 64 != 0) return MHD_EINVAL;
-    if (barrier_mode < 0 || barrier_mode > 2) return MHD_EINVAL;
+    if (barrier_mode < 0 || barrier_mode > 3) return MHD_EINVAL;
     DeviceGuard guard(owning_device(scratch));
+    if (guard.failed) return MHD_ECUDA;
     return measure_exchange((double*)scratch, bytes / sizeof(double), (cudaStream_t)stream, dfma_per_exchange, barrier_mode, smem_gbs) == cudaSuccess ? MHD_OK : MHD_ECUDA;
 }
 
 int mhd_profile_begin(mhd_ctx* c) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     for (int k = 0; k < K_NCLASS; ++k) {
         for (cudaEvent_t ev : c->prof_ev[k]) cudaEventDestroy(ev);
         c->prof_ev[k].clear();
@@ -328,6 +346,7 @@ int mhd_profile_begin(mhd_ctx* c) {
 int mhd_profile_end(mhd_ctx* c, int* counts, double* ms) {
     if (!c || !counts || !ms) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     c->profiling = 0;
     CK(cudaStreamSynchronize(c->st));
     for (int k = 0; k < K_NCLASS; ++k) {
@@ -373,6 +392,8 @@ int mhd_create(mhd_ctx** out, int nx, int ny, int nz, double nu, double eta, dou
     c->st = (cudaStream_t)stream; c->ws = (char*)workspace; c->L = L;
     c->device = owning_device(workspace);
     DeviceGuard guard(c->device);
+    if (guard.failed) { delete c; return MHD_ECUDA; }
+    if (!stream_on_device((cudaStream_t)stream, c->device)) { delete c; return MHD_EINVAL; }
     c->xfuse = use_xfuse(nx, flags);
     c->prof_ev = new (std::nothrow) std::vector<cudaEvent_t>[K_NCLASS];
     if (!c->prof_ev) { delete c; return MHD_ENOMEM; }
@@ -419,6 +440,7 @@ static void invalidate_graph(mhd_ctx* c) {
 int mhd_set_box(mhd_ctx* c, double lx, double ly, double lz) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0) || !isfinite(lx) || !isfinite(ly) || !isfinite(lz))
         return fail(c, MHD_EINVAL, "mhd_set_box: lengths must be finite and > 0");
     const double two_pi = 6.283185307179586476925286766559;
@@ -431,6 +453,7 @@ int mhd_set_box(mhd_ctx* c, double lx, double ly, double lz) {
 int mhd_set_forcing(mhd_ctx* c, const double* fx, const double* fy, const double* fz) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!fx && !fy && !fz) { c->have_forcing = 0; invalidate_graph(c); return MHD_OK; }
     if (!fx || !fy || !fz) return fail(c, MHD_EINVAL, "mhd_set_forcing: give all three components or none");
     if (!(c->flags & MHD_FLAG_FORCING)) return fail(c, MHD_ESTATE, "mhd_set_forcing: context created without MHD_FLAG_FORCING");
@@ -448,6 +471,7 @@ int mhd_set_forcing(mhd_ctx* c, const double* fx, const double* fy, const double
 int mhd_set_forcing_host(mhd_ctx* c, const double* fx, const double* fy, const double* fz) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!fx && !fy && !fz) return mhd_set_forcing(c, nullptr, nullptr, nullptr);
     if (!fx || !fy || !fz) return fail(c, MHD_EINVAL, "mhd_set_forcing_host: give all three components or none");
     if (!(c->flags & MHD_FLAG_FORCING)) return fail(c, MHD_ESTATE, "mhd_set_forcing_host: context created without MHD_FLAG_FORCING");
@@ -461,6 +485,7 @@ int mhd_set_fields(mhd_ctx* c, const double* rho, const double* ux, const double
                    const double* bx, const double* by, const double* bz) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_set_fields: NULL field");
     if (!c->hydro && (!bx || !by || !bz)) return fail(c, MHD_EINVAL, "mhd_set_fields: NULL magnetic field without MHD_FLAG_HYDRO");
     const long long n = c->g.npts;
@@ -481,6 +506,7 @@ int mhd_set_fields_host(mhd_ctx* c, const double* rho, const double* ux, const d
                         const double* bx, const double* by, const double* bz) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_set_fields_host: NULL field");
     if (!c->hydro && (!bx || !by || !bz)) return fail(c, MHD_EINVAL, "mhd_set_fields_host: NULL magnetic field");
     const long long n = c->g.npts;
@@ -496,6 +522,7 @@ int mhd_set_fields_host(mhd_ctx* c, const double* rho, const double* ux, const d
 int mhd_step(mhd_ctx* c, int nsteps) {
     if (!c || nsteps < 0) return c ? fail(c, MHD_EINVAL, "mhd_step: nsteps < 0") : MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_step before mhd_set_fields");
     int done = 0;
     // a launch failure part-way through still leaves `done` completed steps in the state: account for them
@@ -550,6 +577,7 @@ int mhd_step(mhd_ctx* c, int nsteps) {
 int mhd_get_fields(mhd_ctx* c, double* rho, double* ux, double* uy, double* uz, double* bx, double* by, double* bz) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_get_fields: NULL field");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_get_fields before mhd_set_fields");
     const long long n = c->g.npts;
@@ -569,6 +597,7 @@ int mhd_get_fields(mhd_ctx* c, double* rho, double* ux, double* uy, double* uz, 
 int mhd_get_fields_host(mhd_ctx* c, double* rho, double* ux, double* uy, double* uz, double* bx, double* by, double* bz) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!rho || !ux || !uy || !uz) return fail(c, MHD_EINVAL, "mhd_get_fields_host: NULL field");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_get_fields_host before mhd_set_fields");
     const long long n = c->g.npts;
@@ -608,6 +637,7 @@ size_t mhd_state_bytes(const mhd_ctx* c) {
 int mhd_get_state(mhd_ctx* c, void* state, size_t bytes) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!state || bytes < mhd_state_bytes(c)) return fail(c, MHD_EINVAL, "mhd_get_state: buffer missing or too small");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_get_state before mhd_set_fields");
     StateHeader h;
@@ -628,6 +658,7 @@ int mhd_get_state(mhd_ctx* c, void* state, size_t bytes) {
 int mhd_set_state(mhd_ctx* c, const void* state, size_t bytes) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!state || bytes < mhd_state_bytes(c)) return fail(c, MHD_EINVAL, "mhd_set_state: buffer missing or too small");
     StateHeader h;
     CK(cudaMemcpyAsync(&h, state, sizeof(h), cudaMemcpyDeviceToHost, c->st));
@@ -646,6 +677,7 @@ int mhd_set_state(mhd_ctx* c, const void* state, size_t bytes) {
 int mhd_diagnostics(mhd_ctx* c, mhd_diag* out, double* ekin_spec, double* emag_spec, int nshell) {
     if (!c) return MHD_EINVAL;
     DeviceGuard guard(c->device);
+    if (guard.failed) return fail(c, MHD_ECUDA, kGuardFailed);
     if (!out || nshell < 0 || nshell > kMaxShell || (nshell > 0 && (!ekin_spec || !emag_spec)))
         return fail(c, MHD_EINVAL, "mhd_diagnostics: bad argument");
     if (!c->have_fields) return fail(c, MHD_ESTATE, "mhd_diagnostics before mhd_set_fields");
@@ -754,14 +786,16 @@ PlaneGeom plane_geom(int n) {
     return g;
 }
 struct FftLayout { size_t twx, twy, twz, work, ring, counters, total; };
-FftLayout make_fft_layout(int nx, int ny, int nz, int batch) {
+// with_ring: also the plane pipeline's ring and counters (only a plan that will use MHD_FFT_PLANE_PIPELINE pays for them);
+// the layout without them is a prefix of the layout with them
+FftLayout make_fft_layout(int nx, int ny, int nz, int batch, bool with_ring) {
     FftLayout L;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes, 256); return at; };
     L.twx = take(sizeof(double2) * nx); L.twy = take(sizeof(double2) * ny); L.twz = take(sizeof(double2) * nz);
     L.work = take(sizeof(double2) * (size_t)(nx / 2 + 1) * ny * nz * batch);
     L.ring = L.counters = o;
-    if (planefft_supported(nx, ny)) {
+    if (with_ring && planefft_supported(nx, ny)) {
         const PlaneGeom g = plane_geom(nx);
         L.ring = take(sizeof(double2) * (size_t)g.ring_slots * g.group * ny * g.pitch);
         L.counters = take(planefft_counter_bytes((long long)batch * nz, g.group));
@@ -787,25 +821,35 @@ extern "C" {
 
 size_t mhd_fft_workspace_bytes(int nx, int ny, int nz, int batch) {
     if (!fft_dims_ok(nx, ny, nz, batch)) return 0;
-    return make_fft_layout(nx, ny, nz, batch).total;
+    return make_fft_layout(nx, ny, nz, batch, false).total;
+}
+
+size_t mhd_fft_plane_workspace_bytes(int nx, int ny, int nz, int batch) {
+    if (!fft_dims_ok(nx, ny, nz, batch) || !planefft_supported(nx, ny)) return 0;
+    return make_fft_layout(nx, ny, nz, batch, true).total;
 }
 
 int mhd_fft_plan_create(mhd_fft_plan** out, int nx, int ny, int nz, int batch, void* workspace, size_t bytes, void* stream) {
     if (!out) return MHD_EINVAL;
     *out = nullptr;
     if (!fft_dims_ok(nx, ny, nz, batch)) return MHD_EINVAL;
-    const FftLayout L = make_fft_layout(nx, ny, nz, batch);
+    FftLayout L = make_fft_layout(nx, ny, nz, batch, false);
     if (!workspace || bytes < L.total || ((size_t)workspace & 255u)) return MHD_EINVAL;
+    const bool with_ring = planefft_supported(nx, ny) && bytes >= make_fft_layout(nx, ny, nz, batch, true).total;
+    if (with_ring) L = make_fft_layout(nx, ny, nz, batch, true);
     mhd_fft_plan* p = new (std::nothrow) mhd_fft_plan();
     if (!p) return MHD_ENOMEM;
     p->err[0] = 0;
     p->device = owning_device(workspace);
     DeviceGuard guard(p->device);
+    if (guard.failed) { delete p; return MHD_ECUDA; }
+    if (!stream_on_device((cudaStream_t)stream, p->device)) { delete p; return MHD_EINVAL; }
     p->nx = nx; p->ny = ny; p->nz = nz; p->batch = batch; p->nxh = nx / 2 + 1; p->st = (cudaStream_t)stream;
     char* ws = (char*)workspace;
     p->twx = (double2*)(ws + L.twx); p->twy = (double2*)(ws + L.twy); p->twz = (double2*)(ws + L.twz); p->work = (double2*)(ws + L.work);
     p->plane = 0;              // default: three sweeps (faster on B200, see mhd_fft_plan_set_mode in mhd.h)
-    if (planefft_supported(nx, ny)) {
+    p->ring = nullptr; p->counters = nullptr;
+    if (with_ring) {
         const PlaneGeom g = plane_geom(nx);
         p->group = g.group; p->ring_slots = g.ring_slots; p->lag = g.lag; p->pitch = g.pitch;
         p->ring = (double2*)(ws + L.ring); p->counters = (unsigned*)(ws + L.counters);
@@ -829,6 +873,10 @@ void mhd_fft_plan_destroy(mhd_fft_plan* p) { delete p; }
 int mhd_fft_plan_set_mode(mhd_fft_plan* p, int mode) {
     if (!p || (mode != MHD_FFT_THREE_SWEEP && mode != MHD_FFT_PLANE_PIPELINE)) return MHD_EINVAL;
     if (mode == MHD_FFT_PLANE_PIPELINE && !planefft_supported(p->nx, p->ny)) return MHD_EINVAL;
+    if (mode == MHD_FFT_PLANE_PIPELINE && !p->ring) {
+        snprintf(p->err, sizeof(p->err), "mhd_fft_plan_set_mode: the plan's workspace has no ring (create it with mhd_fft_plane_workspace_bytes)");
+        return MHD_EINVAL;
+    }
     p->plane = (mode == MHD_FFT_PLANE_PIPELINE) ? 1 : 0;
     return MHD_OK;
 }
@@ -838,6 +886,7 @@ const char* mhd_fft_last_error(const mhd_fft_plan* p) { return p ? p->err : ""; 
 int mhd_fft_r2c(mhd_fft_plan* p, const double* in, double* out) {
     if (!p || !in || !out) return MHD_EINVAL;
     DeviceGuard guard(p->device);
+    if (guard.failed) { snprintf(p->err, sizeof(p->err), "%s", kGuardFailed); return MHD_ECUDA; }
     double2* o = (double2*)out;
     const long long plane = (long long)p->ny * p->nxh, vol = plane * p->nz;
     AxisArgs a;
@@ -869,6 +918,7 @@ int mhd_fft_r2c(mhd_fft_plan* p, const double* in, double* out) {
 int mhd_fft_c2r(mhd_fft_plan* p, const double* in, double* out) {
     if (!p || !in || !out) return MHD_EINVAL;
     DeviceGuard guard(p->device);
+    if (guard.failed) { snprintf(p->err, sizeof(p->err), "%s", kGuardFailed); return MHD_ECUDA; }
     const double2* src = (const double2*)in;
     const long long plane = (long long)p->ny * p->nxh, vol = plane * p->nz;
     AxisArgs a;

@@ -47,7 +47,27 @@ __global__ void __launch_bounds__(256) peak_smem_kernel(double* __restrict__ out
 //          bytes = 32 x 16 per thread per iteration.
 #define MHD_PAD8(e) ((e) + ((e) >> 3))
 // MODE 0: write, barrier, read, barrier; 1: barrier, write, barrier, read (the shipped x passes); 2: two buffers per set used
-// alternately, ONE barrier per exchange (write, barrier, read)
+// alternately, ONE barrier per exchange (write, barrier, read); 3: no shared memory and no barrier at all -- the same 16 complex
+// values per thread are exchanged by an 8 x 8 register transpose among the 8 lanes of a warp octet (three __shfl_xor_sync
+// butterfly rounds, 4 of the 8 values of a set per round): the most a warp-shuffle exchange could do for a radix-8 pass, as
+// an upper bound for the north-star's "warp-shuffle butterflies" question (a 64-thread team would still need one
+// shared-memory exchange on top, because its transposition spans two warps)
+__device__ __forceinline__ double2 shfl_xor_c(double2 x, int mask) {
+    x.x = __shfl_xor_sync(0xffffffffu, x.x, mask);
+    x.y = __shfl_xor_sync(0xffffffffu, x.y, mask);
+    return x;
+}
+// one butterfly round of the octet transpose: lanes whose bit R is 0 give away the values whose index has bit R set, and v.v.
+template <int R> __device__ __forceinline__ void transpose_round(double2 (&v)[8], bool hi) {
+#pragma unroll
+    for (int q0 = 0; q0 < 8; ++q0) {
+        if (q0 & (1 << R)) continue;
+        const int q1 = q0 | (1 << R);
+        const double2 send = hi ? v[q0] : v[q1];
+        const double2 recv = shfl_xor_c(send, 1 << R);
+        if (hi) v[q0] = recv; else v[q1] = recv;
+    }
+}
 template <int REPS, int MODE>
 __global__ void __launch_bounds__(256, 1) peak_exchange_kernel(double* __restrict__ out, int iters, double a, double b) {
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -65,6 +85,13 @@ __global__ void __launch_bounds__(256, 1) peak_exchange_kernel(double* __restric
                 v[q].x = fma(v[q].x, a, b); v[q].y = fma(v[q].y, a, -b);
                 w[q].x = fma(w[q].x, a, b); w[q].y = fma(w[q].y, a, -b);
             }
+        if (MODE == 3) {
+            const int lane = threadIdx.x & 31;
+            transpose_round<0>(v, lane & 1); transpose_round<0>(w, lane & 1);
+            transpose_round<1>(v, lane & 2); transpose_round<1>(w, lane & 2);
+            transpose_round<2>(v, lane & 4); transpose_round<2>(w, lane & 4);
+            continue;
+        }
         double2* const A = base + ((MODE == 2) ? (it & 1) * 1280 : 0);
         double2* const B = A + 640;
         if (MODE == 1) asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
@@ -92,8 +119,8 @@ cudaError_t measure_exchange(double* scratch, size_t scratch_doubles, cudaStream
     const int reps = dfma_per_exchange / 32;
     void (*kern)(double*, int, double, double) = nullptr;
 #define MHD_EXCH(R_)                                                                              \
-    case R_: kern = mode == 0 ? peak_exchange_kernel<R_, 0> : mode == 1 ? peak_exchange_kernel<R_, 1> : peak_exchange_kernel<R_, 2>; break;
-    if (mode < 0 || mode > 2) return cudaErrorInvalidValue;
+    case R_: kern = mode == 0 ? peak_exchange_kernel<R_, 0> : mode == 1 ? peak_exchange_kernel<R_, 1> : mode == 2 ? peak_exchange_kernel<R_, 2> : peak_exchange_kernel<R_, 3>; break;
+    if (mode < 0 || mode > 3) return cudaErrorInvalidValue;
     switch (reps) {
         MHD_EXCH(0) MHD_EXCH(2) MHD_EXCH(4) MHD_EXCH(6) MHD_EXCH(8)
         default: return cudaErrorInvalidValue;

@@ -164,7 +164,9 @@ __global__ void __launch_bounds__(XCfg2<N>::THREADS, 1) xfused_kernel(XFusedArgs
                 // the staging area of this group is free again: the team has passed a barrier since reading it (a one-thread
                 // team needs none).  Refill it with the same group of the team's next row.
                 if constexpr (PL::NP == 1 && TP > 1) team_sync<TP>(team);
-                if (i == 0 && ok && row + row_stride < a.nrows) stage_group(row + row_stride, grp);
+                // (the team barrier orders the other threads' ld.shared before this point; the proxy fence orders those
+                // generic-proxy reads before the async-proxy writes of the bulk copies issued next)
+                if (i == 0 && ok && row + row_stride < a.nrows) { fence_proxy_async(); stage_group(row + row_stride, grp); }
             }
             const double s = a.scale;
             // last-pass outputs: register m*RL + q holds x = i + TP*m + q*(N/RL) = i + TP*(m + q*(E/RL))
@@ -480,7 +482,8 @@ __global__ void __launch_bounds__(XRowStagedCfg<N>::THREADS, 1) xrows_inv_staged
         const bool oku = u < nunits;
         const bool oka = oku && 2 * u < npairs, okb = oku && 2 * u + 1 < npairs;
         // every thread of the team has finished reading buffer b^1 (it passed the team barriers of the previous transform)
-        if (i == 0 && u + stride < nunits) stage_unit(u + stride, b ^ 1);
+        // (generic-proxy reads, then async-proxy writes of the same bytes: proxy fence in the issuing thread)
+        if (i == 0 && u + stride < nunits) { fence_proxy_async(); stage_unit(u + stride, b ^ 1); }
         if (oku) { mbar_wait(&mbar[b], (phase >> b) & 1u); phase ^= 1u << b; }
         const cplx* __restrict__ A0 = stage + (size_t)b * 4 * pitch;
         const cplx* __restrict__ A1 = A0 + pitch;

@@ -26,6 +26,7 @@ EXPORTS = [
     "mhd_state_bytes", "mhd_get_state", "mhd_set_state",
     "mhd_get_fields", "mhd_get_fields_host", "mhd_diagnostics", "mhd_strerror", "mhd_last_error",
     "mhd_fft_workspace_bytes", "mhd_fft_plan_create", "mhd_fft_r2c", "mhd_fft_c2r", "mhd_fft_plan_destroy", "mhd_fft_last_error", "mhd_fft_plan_set_mode",
+    "mhd_fft_plane_workspace_bytes",
     "mhd_fft_c2r_static",
     "mhd_launch_count", "mhd_profile_kernel_count", "mhd_profile_kernel_name", "mhd_profile_begin", "mhd_profile_end",
     "mhd_measure_peaks", "mhd_measure_exchange",
@@ -81,6 +82,8 @@ def lib():
         L.mhd_last_error.argtypes = [_vp]
         L.mhd_fft_workspace_bytes.restype = C.c_size_t
         L.mhd_fft_workspace_bytes.argtypes = [C.c_int] * 4
+        L.mhd_fft_plane_workspace_bytes.restype = C.c_size_t
+        L.mhd_fft_plane_workspace_bytes.argtypes = [C.c_int] * 4
         L.mhd_fft_plan_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.c_size_t, _vp]
         L.mhd_fft_r2c.argtypes = [_vp, _vp, _vp]
         L.mhd_fft_c2r.argtypes = [_vp, _vp, _vp]
@@ -343,14 +346,18 @@ class FftPlan:
     def stream(self):
         return self._stream
 
-    def __init__(self, nx, ny, nz, batch, stream=None, device="cuda:0", mode=FFT_THREE_SWEEP):
+    def __init__(self, nx, ny, nz, batch, stream=None, device="cuda:0", mode=FFT_THREE_SWEEP, plane_workspace=False):
+        """plane_workspace (implied by mode=FFT_PLANE_PIPELINE): size the workspace for the plane pipeline's ring too
+        (mhd_fft_plane_workspace_bytes), so that set_mode(FFT_PLANE_PIPELINE) is allowed later; the default plan does not pay."""
         torch = _torch()
         L = lib()
         self.nx, self.ny, self.nz, self.batch = int(nx), int(ny), int(nz), int(batch)
         self.device = torch.device(device)
-        nbytes = L.mhd_fft_workspace_bytes(self.nx, self.ny, self.nz, self.batch)
+        want_ring = bool(plane_workspace) or mode == FFT_PLANE_PIPELINE
+        sizer = L.mhd_fft_plane_workspace_bytes if want_ring else L.mhd_fft_workspace_bytes
+        nbytes = sizer(self.nx, self.ny, self.nz, self.batch)
         if nbytes == 0:
-            raise MhdError(EINVAL, "mhd_fft_workspace_bytes", f"unsupported size {nx}x{ny}x{nz} batch {batch}")
+            raise MhdError(EINVAL, sizer.__name__, f"unsupported size {nx}x{ny}x{nz} batch {batch}")
         with torch.cuda.device(self.device):
             self._ws = torch.empty(int(nbytes) + 256, dtype=torch.uint8, device=self.device)
             off = (-self._ws.data_ptr()) % 256
@@ -371,7 +378,7 @@ class FftPlan:
         """FFT_THREE_SWEEP (default) or FFT_PLANE_PIPELINE (x and y passes through an L2-resident ring; square planes 64..512)"""
         rc = lib().mhd_fft_plan_set_mode(self._h, int(mode))
         if rc != OK:
-            raise MhdError(rc, "mhd_fft_plan_set_mode")
+            raise MhdError(rc, "mhd_fft_plan_set_mode", lib().mhd_fft_last_error(self._h).decode())
 
     def r2c(self, real, out=None):
         torch = _torch()

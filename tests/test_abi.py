@@ -119,10 +119,13 @@ def test_peaks_probe_rejects_bad_arguments(lib):
     assert lib.mhd_measure_exchange(None, 1 << 23, None, 192, 1, C.byref(s)) == mhd.EINVAL
     assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 100, 1, C.byref(s)) == mhd.EINVAL     # not a multiple of 64
     assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 320, 1, C.byref(s)) == mhd.EINVAL
-    assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 192, 3, C.byref(s)) == mhd.EINVAL     # no such barrier mode
+    assert lib.mhd_measure_exchange(C.c_void_p(256), 1 << 23, None, 192, 4, C.byref(s)) == mhd.EINVAL     # no such exchange mode
     assert lib.mhd_fft_last_error(None) == b""
     assert lib.mhd_fft_plan_set_mode(None, 0) == mhd.EINVAL
-    # the plane pipeline needs a ring + counters in the plan workspace only for square planes of 64..512
-    assert lib.mhd_fft_workspace_bytes(512, 512, 8, 1) > lib.mhd_fft_workspace_bytes(512, 256, 8, 1) * 2 - (1 << 20)
-    ring = lib.mhd_fft_workspace_bytes(256, 256, 8, 1) - (16 * 256 * 3 + 16 * 129 * 256 * 8)
+    # the plane pipeline's ring + counters are paid for only by a plan that asks for them, and only exist for square planes of 64..512
+    plain = lib.mhd_fft_workspace_bytes(256, 256, 8, 1)
+    assert 16 * 129 * 256 * 8 <= plain < 16 * 129 * 256 * 8 + 16 * 256 * 3 + 4096
+    ring = lib.mhd_fft_plane_workspace_bytes(256, 256, 8, 1) - plain
     assert 15e6 < ring < 30e6                        # 5 slots of about 4 MB
+    assert lib.mhd_fft_plane_workspace_bytes(512, 256, 8, 1) == 0 and lib.mhd_fft_plane_workspace_bytes(32, 32, 8, 1) == 0
+    assert lib.mhd_fft_plane_workspace_bytes(100, 100, 8, 1) == 0

@@ -202,6 +202,31 @@ def test_solver_runs_while_the_current_stream_and_device_context_differ(gpu):
     assert bool((junk == 7.0).all())
 
 
+def test_solver_on_a_second_gpu_while_the_first_is_current(gpu):
+    """include/mhd.h: contexts on different devices of one process are independent, and every call makes the device that
+    owns the workspace current for its own duration.  A solver created on cuda:1 and driven while cuda:0 is current must
+    equal a cuda:0 run bit for bit and leave cuda:0 current; a stream that lives on the other GPU is refused at create.
+    Needs two GPUs (the round's boxes have one: skipped there, with the reason)."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip(f"needs 2 GPUs, this box has {torch.cuda.device_count()}")
+    cfg = inputs.config1()
+    torch.cuda.set_device(0)
+    a = gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, device="cuda:0")
+    a.set_fields(*[torch.from_numpy(x).to("cuda:0") for x in cfg.arrays()]); a.step(12)
+    b = gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, device="cuda:1")
+    assert torch.cuda.current_device() == 0
+    b.set_fields(*[torch.from_numpy(x).to("cuda:1") for x in cfg.arrays()]); b.step(12)
+    assert torch.cuda.current_device() == 0
+    for x, y in zip(a.get_fields(), b.get_fields()):
+        assert y.device.index == 1 and torch.equal(x.cpu(), y.cpu())
+    da, db = a.diagnostics(8), b.diagnostics(8)
+    assert da["ekin"] == db["ekin"] and np.array_equal(da["ekin_spec"], db["ekin_spec"])
+    with pytest.raises(gpu.MhdError) as e:
+        gpu.Solver(cfg.nx, cfg.ny, cfg.nz, cfg.nu, cfg.eta, cfg.cs, cfg.dt, device="cuda:1", stream=torch.cuda.Stream(device="cuda:0"))
+    assert e.value.code == gpu.EINVAL
+
+
 @pytest.mark.parametrize("integrator", [0, 1])
 def test_exact_resume_is_bit_identical(gpu, integrator):
     """mhd_get_state / mhd_set_state: a run interrupted after 5 steps and continued in a fresh
@@ -246,5 +271,10 @@ def test_onchip_probes_are_consistent(gpu):
         ex = gpu.measure_exchange(192, "cuda:0", mode)
         assert 0.5 * smem < ex < 1.02 * smem, (mode, ex, smem)
     assert gpu.measure_exchange(0, "cuda:0") >= 0.95 * gpu.measure_exchange(256, "cuda:0")     # FP64 work never speeds the exchange up
+    shuffle = gpu.measure_exchange(192, "cuda:0", 3)                 # mode 3: warp-shuffle octet transpose, no shared memory
+    print(f"exchange probe at 192 DFMA: shared memory {ex:.0f} GB/s-equivalent, warp shuffle {shuffle:.0f}")
+    assert 1e3 < shuffle < 4.0 * smem
     with pytest.raises(gpu.MhdError):
         gpu.measure_exchange(100, "cuda:0")
+    with pytest.raises(gpu.MhdError):
+        gpu.measure_exchange(192, "cuda:0", 4)

@@ -65,6 +65,13 @@ def test_plane_pipelined_xy_pass_against_the_oracle(gpu, ref, shape, batch):
     check(gpu, ref, shape, batch, mode=gpu.FFT_PLANE_PIPELINE)
     with pytest.raises(gpu.MhdError):
         gpu.FftPlan(32, 16, 8, 1, mode=gpu.FFT_PLANE_PIPELINE)
+    # the ring is paid for only on request: a default-sized plan may not switch, one sized by mhd_fft_plane_workspace_bytes may
+    plain = gpu.FftPlan(64, 64, 8, 1)
+    with pytest.raises(gpu.MhdError, match="no ring"):
+        plain.set_mode(gpu.FFT_PLANE_PIPELINE)
+    ringed = gpu.FftPlan(64, 64, 8, 1, plane_workspace=True)
+    ringed.set_mode(gpu.FFT_PLANE_PIPELINE)
+    ringed.set_mode(gpu.FFT_THREE_SWEEP)
 
 
 @pytest.mark.parametrize("n,mode", [(256, 0), (512, 0), (768, 0), (256, 1), (512, 1)])
